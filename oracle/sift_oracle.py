@@ -1,0 +1,418 @@
+"""CPU oracle for SIFT's decode + block-sparse prefill attention (arxiv/paper_2606_09441).
+
+TEST INFRASTRUCTURE ONLY.  Only ``tests/``, ``__graft_entry__.smoke()`` and the
+``cpu_baseline`` / ``--impl reference`` legs of ``bench.py`` may import this file.  It
+shares no code with the CUDA path (``paper_2606_09441_b200/``) and does not import it;
+the two only ever see the same seeded input arrays.
+
+What it is: the plain definitions, written out.
+  Part 1  ``expand_mask_rows``   -- the boolean mask the two bit vectors stand for
+                                    (Fig 6; L201-203 sec 4.1; L209 sec 4.2).
+  Part 2  ``attention_rows``     -- masked two-pass softmax attention, one row block at a time
+                                    (north_star: "expands the bit vectors into an explicit boolean
+                                    mask and runs fp32 masked softmax attention"; fp64 on request).
+  Part 3  ``decode_metadata``    -- the decode kernel's output, pass 1 count -> offsets -> pass 2 fill,
+                                    CA entries then LA entries, global coordinates
+                                    (sec 5.1), in the container "MD-v1"
+                                    (SURVEY.md 8(c) Part 3; the paper fixes no container).
+  Sizes   ``la_vector_bytes`` .. -- PAPER.md:L213 sec 4.3 and Table 1 (L311-321).
+
+Readings of the paper where it is silent or garbled are listed in DESIGN.md section 3
+(A1..A26 of SURVEY.md 8(c)); the ones used here are cited inline.
+
+Pins (tests/test_oracle_pins.py): byte patterns from the enumeration printed at L203, the
+P=8 -> 36/8 bits example (L213), all of Table 1, all-ones == dense causal, CA cleared ==
+block diagonal + dense query, brute-force fp64 softmax on tiny inputs, the torch SDPA
+special case, metadata -> mask round trip, reorder invariance.
+Parity unpinned by the paper: the MD-v1 *container layout* (our definition; pinned only by
+the round trip).
+"""
+from __future__ import annotations
+
+import math
+from typing import Callable, Dict, List, Optional, Sequence, Tuple
+
+import numpy as np
+import torch
+
+VecFn = Callable[[int, int, int], np.ndarray]  # (layer, head, doc position) -> uint8 vector
+
+
+# ------------------------------------------------------------------------------------------
+# Sizes (Table 1)
+# ------------------------------------------------------------------------------------------
+
+def pages(doc_len: int, tile: int) -> int:
+    """P = ceil(L / T)."""
+    return -(-doc_len // tile)
+
+
+def la_vector_bits(p: int) -> int:
+    """Lower triangle of a PxP tile grid incl. the diagonal: P(P+1)/2 bits (L201-203, L213)."""
+    return p * (p + 1) // 2
+
+
+def la_vector_bytes(p: int) -> int:
+    """ceil(P(P+1)/(2*8)) bytes (L213)."""
+    return -(-la_vector_bits(p) // 8)
+
+
+def ca_vector_bits(doc_len: int, tile: int, gran: int) -> int:
+    """Paper (gran == tile): one bit per KV page -> P bits (L209, L213).
+    BASELINE.json configs (gran == 1): one bit per key token -> L bits (reading A4)."""
+    return -(-doc_len // gran)
+
+
+def ca_vector_bytes(doc_len: int, tile: int, gran: int) -> int:
+    return -(-ca_vector_bits(doc_len, tile, gran) // 8)
+
+
+def sift_storage_bits(n_layers: int, n_heads: int, n_docs: int, p: int) -> int:
+    """Unpadded bits for one prompt, page-granular CA (Table 1 reading: per q-head, A7)."""
+    return n_layers * n_heads * n_docs * (la_vector_bits(p) + p)
+
+
+# ------------------------------------------------------------------------------------------
+# Bit access ("packed MSB-first, enumerated row-major in the lower triangle")
+# ------------------------------------------------------------------------------------------
+
+def get_bit(vec: np.ndarray, n: int) -> int:
+    return (int(vec[n >> 3]) >> (7 - (n & 7))) & 1
+
+
+def la_bit_index(i: int, j: int) -> int:
+    """(0,0),(1,0),(1,1),(2,0)...: row i starts after 1+2+...+i = i(i+1)/2 bits."""
+    assert 0 <= j <= i
+    return i * (i + 1) // 2 + j
+
+
+def la_tile_bit(vec: np.ndarray, i: int, j: int) -> int:
+    return get_bit(vec, la_bit_index(i, j))
+
+
+def read_bits(vec: np.ndarray, nbits: int) -> np.ndarray:
+    """get_bit applied to n = 0..nbits-1 (same formula, element-wise). Padding bits beyond
+    nbits are never looked at (reading A6)."""
+    n = np.arange(nbits, dtype=np.int64)
+    return ((vec[n >> 3].astype(np.int64) >> (7 - (n & 7))) & 1).astype(bool)
+
+
+# ------------------------------------------------------------------------------------------
+# Part 1: the mask
+# ------------------------------------------------------------------------------------------
+
+def segment_of(row: int, doc_offsets: Sequence[int]) -> int:
+    """Index of the document holding global row `row`; len(doc_offsets)-1 (= D) for the user query."""
+    d_total = len(doc_offsets) - 1
+    for d in range(d_total):
+        if doc_offsets[d] <= row < doc_offsets[d + 1]:
+            return d
+    return d_total
+
+
+def expand_mask_rows(doc_offsets: Sequence[int], query_len: int, tile: int, gran: int,
+                     la_vecs: Sequence[np.ndarray], ca_vecs: Sequence[np.ndarray],
+                     rows: Sequence[int]) -> np.ndarray:
+    """bool [len(rows), N] for one (layer, head). la_vecs[d] / ca_vecs[d] are that head's vectors.
+
+    Rule (SURVEY.md 8(c) Part 1):
+      1. k > q                     -> False   (causal; L201 "lower triangular ... due to causality")
+      2. q in the user query       -> True    (L149 "query submatrix is always recomputed"; L243)
+      3. q in doc d, k in doc d':
+           d' == d -> LA_d bit of tile (floor(r/T), floor(c/T))          (L201-203)
+           d' <  d -> CA_d' bit floor(c/G)                               (L177, L209; A16: every d'<d)
+    """
+    off = [int(x) for x in doc_offsets]
+    n_docs = len(off) - 1
+    n = off[-1] + query_len
+    cross_allowed = [read_bits(ca_vecs[d], ca_vector_bits(off[d + 1] - off[d], tile, gran)) for d in range(n_docs)]
+    out = np.zeros((len(rows), n), dtype=bool)
+    for ri, q in enumerate(rows):
+        q = int(q)
+        d = segment_of(q, off)
+        if d == n_docs:                      # user query row: dense causal
+            out[ri, : q + 1] = True
+            continue
+        for dp in range(d):                  # earlier documents: per-key CA bit
+            length = off[dp + 1] - off[dp]
+            c = np.arange(length)
+            out[ri, off[dp]: off[dp + 1]] = cross_allowed[dp][c // gran]
+        r = q - off[d]
+        i = r // tile
+        for j in range(i + 1):               # own document: LA tile bit, then causality
+            if la_tile_bit(la_vecs[d], i, j):
+                c0 = off[d] + j * tile
+                c1 = min(off[d] + (j + 1) * tile, off[d + 1])
+                out[ri, c0: min(c1, q + 1)] = True
+    return out
+
+
+# ------------------------------------------------------------------------------------------
+# Part 2: masked softmax attention (two-pass, no tiling, no online softmax)
+# ------------------------------------------------------------------------------------------
+
+def attention_rows(q_rows: torch.Tensor, k_all: torch.Tensor, v_all: torch.Tensor, mask: np.ndarray,
+                   scale: float, dtype: torch.dtype = torch.float32) -> Tuple[torch.Tensor, torch.Tensor]:
+    """q_rows [R,d], k_all/v_all [N,d] (any float dtype; widened exactly), mask bool [R,N].
+    Returns O [R,d] and LSE [R] in `dtype`.
+      s_k = scale * <q, k>;  m = max_k s_k;  l = sum_k exp(s_k - m);
+      O = sum_k exp(s_k - m) v_k / l;  LSE = m + ln l   (natural log of scaled logits, A15).
+    A row with no allowed key gives O = 0, LSE = -inf (A13)."""
+    qf, kf, vf = q_rows.to(dtype), k_all.to(dtype), v_all.to(dtype)
+    m_t = torch.from_numpy(np.ascontiguousarray(mask))
+    s = (qf @ kf.T) * scale
+    s = torch.where(m_t, s, torch.full_like(s, -math.inf))
+    mx = s.max(dim=1).values
+    empty = ~m_t.any(dim=1)
+    mx_safe = torch.where(empty, torch.zeros_like(mx), mx)
+    p = torch.exp(s - mx_safe[:, None])          # masked entries: exp(-inf) = 0
+    l = p.sum(dim=1)
+    o = (p @ vf) / torch.where(empty, torch.ones_like(l), l)[:, None]
+    lse = torch.where(empty, torch.full_like(mx, -math.inf), mx_safe + torch.log(torch.where(empty, torch.ones_like(l), l)))
+    return o, lse
+
+
+def kv_head_of(h: int, n_q_heads: int, n_kv_heads: int) -> int:
+    """Contiguous GQA groups: kv(h) = floor(h / (Hq/Hkv))  (A8)."""
+    return h // (n_q_heads // n_kv_heads)
+
+
+def sift_attention_rows(q: torch.Tensor, k: torch.Tensor, v: torch.Tensor, head: int,
+                        doc_offsets: Sequence[int], query_len: int, tile: int, gran: int,
+                        la_vecs: Sequence[np.ndarray], ca_vecs: Sequence[np.ndarray], rows: Sequence[int],
+                        scale: Optional[float] = None, dtype: torch.dtype = torch.float32,
+                        block: int = 64) -> Tuple[torch.Tensor, torch.Tensor]:
+    """SIFT prefill attention for q-head `head` on the given global rows.
+    q [N,Hq,d], k,v [N,Hkv,d].  The mask is materialised `block` rows at a time."""
+    n, hq, d = q.shape
+    hkv = k.shape[1]
+    if scale is None:
+        scale = 1.0 / math.sqrt(d)           # A14
+    kvh = kv_head_of(head, hq, hkv)
+    rows = [int(r) for r in rows]
+    outs, lses = [], []
+    for b0 in range(0, len(rows), block):
+        rb = rows[b0: b0 + block]
+        mask = expand_mask_rows(doc_offsets, query_len, tile, gran, la_vecs, ca_vecs, rb)
+        kmax = max(rb) + 1                   # keys after the last row of the block are causally dead
+        o, lse = attention_rows(q[rb, head, :], k[:kmax, kvh, :], v[:kmax, kvh, :], mask[:, :kmax], scale, dtype)
+        outs.append(o)
+        lses.append(lse)
+    if not outs:
+        return torch.zeros((0, d), dtype=dtype), torch.zeros((0,), dtype=dtype)
+    return torch.cat(outs), torch.cat(lses)
+
+
+def dense_causal_rows(q: torch.Tensor, k: torch.Tensor, v: torch.Tensor, head: int, rows: Sequence[int],
+                      scale: Optional[float] = None, dtype: torch.dtype = torch.float32,
+                      block: int = 64) -> Tuple[torch.Tensor, torch.Tensor]:
+    """Plain dense causal attention (the "Full Recompute" comparator)."""
+    n, hq, d = q.shape
+    if scale is None:
+        scale = 1.0 / math.sqrt(d)
+    kvh = kv_head_of(head, hq, k.shape[1])
+    rows = [int(r) for r in rows]
+    outs, lses = [], []
+    for b0 in range(0, len(rows), block):
+        rb = rows[b0: b0 + block]
+        kmax = max(rb) + 1
+        mask = np.arange(kmax)[None, :] <= np.asarray(rb)[:, None]
+        o, lse = attention_rows(q[rb, head, :], k[:kmax, kvh, :], v[:kmax, kvh, :], mask, scale, dtype)
+        outs.append(o)
+        lses.append(lse)
+    return torch.cat(outs), torch.cat(lses)
+
+
+def brute_force_row(q_row: np.ndarray, k_all: np.ndarray, v_all: np.ndarray, allowed: Sequence[int],
+                    scale: float) -> Tuple[np.ndarray, float]:
+    """Pure-Python fp64 loops, one row; for tiny pins only."""
+    d = len(q_row)
+    if len(allowed) == 0:
+        return np.zeros(d), -math.inf
+    s = []
+    for kk in allowed:
+        acc = 0.0
+        for t in range(d):
+            acc += float(q_row[t]) * float(k_all[kk][t])
+        s.append(acc * scale)
+    m = max(s)
+    w = [math.exp(x - m) for x in s]
+    l = sum(w)
+    o = np.zeros(d)
+    for wi, kk in zip(w, allowed):
+        for t in range(d):
+            o[t] += wi * float(v_all[kk][t])
+    return o / l, m + math.log(l)
+
+
+# ------------------------------------------------------------------------------------------
+# Part 3: metadata decode (MD-v1)
+# ------------------------------------------------------------------------------------------
+
+def tile_tables(doc_offsets: Sequence[int], query_len: int, tile: int) -> Dict[str, np.ndarray]:
+    """Doc-relative tiles (A2): tile (d,i) covers rows off[d]+iT .. ; the query is segment D.
+    Returns P[D+1], tile_base[D+2], tile_seg[NT], tile_row0[NT], tile_rows[NT]."""
+    off = [int(x) for x in doc_offsets]
+    n_docs = len(off) - 1
+    seg_len = [off[d + 1] - off[d] for d in range(n_docs)] + [query_len]
+    seg_off = off[:-1] + [off[-1]]
+    p = [pages(x, tile) for x in seg_len]
+    base = [0]
+    for x in p:
+        base.append(base[-1] + x)
+    seg, row0, nrows = [], [], []
+    for d in range(n_docs + 1):
+        for i in range(p[d]):
+            seg.append(d)
+            row0.append(seg_off[d] + i * tile)
+            nrows.append(min(tile, seg_len[d] - i * tile))
+    return {"P": np.asarray(p, np.int32), "tile_base": np.asarray(base, np.int32), "NT": base[-1],
+            "tile_seg": np.asarray(seg, np.int32), "tile_row0": np.asarray(row0, np.int32),
+            "tile_rows": np.asarray(nrows, np.int32)}
+
+
+def cross_capacity(doc_offsets: Sequence[int], gran: int) -> int:
+    """ceil(off[D]/G) rounded up to a multiple of 128 (SURVEY.md 8(c) MD-v1)."""
+    n = -(-int(doc_offsets[-1]) // gran)
+    return -(-n // 128) * 128
+
+
+def local_capacity(tt: Dict[str, np.ndarray]) -> int:
+    """sum_d P_d(P_d+1)/2 over documents + sum over query tiles (global id t) of (t+1)."""
+    p, base = tt["P"], tt["tile_base"]
+    n_docs = len(p) - 1
+    cap = sum(int(p[d]) * (int(p[d]) + 1) // 2 for d in range(n_docs))
+    for t in range(int(base[n_docs]), int(base[n_docs + 1])):
+        cap += t + 1
+    return cap
+
+
+def decode_metadata(doc_offsets: Sequence[int], query_len: int, tile: int, gran: int,
+                    n_layers: int, n_heads: int, la_vec: VecFn, ca_vec: VecFn,
+                    layers: Optional[Sequence[int]] = None) -> Dict[str, np.ndarray]:
+    """Follows PAPER.md:L241-245: pass 1 counts marked CA and LA bits per (head, M-block)
+    (query M-blocks: the number of causal N-blocks, L243); offsets = prefix sums of the counts;
+    pass 2 scans CA then LA and writes the indices, offset to global coordinates, at their
+    designated offset.  Container MD-v1: the CA entries of a document are a prefix of one
+    per-head list (``cross_ptr``), instead of being replicated into every M-block's list;
+    ``paper_view`` rebuilds the per-(head, M-block) list of L239.
+
+    cross_idx: G == 1 -> global key row off[d']+c ; G == tile -> global tile id tile_base[d']+b.
+    Entries of cross_idx at or beyond cross_ptr[..., D] and of local_idx beyond local_ptr[..., NT]
+    are unspecified (-1 here; never compared)."""
+    off = [int(x) for x in doc_offsets]
+    n_docs = len(off) - 1
+    tt = tile_tables(off, query_len, tile)
+    nt, base, p = int(tt["NT"]), tt["tile_base"], tt["P"]
+    ccap, lcap = cross_capacity(off, gran), local_capacity(tt)
+    lay = list(range(n_layers)) if layers is None else list(layers)
+    cross_ptr = np.zeros((n_layers, n_heads, n_docs + 1), np.int32)
+    cross_idx = np.full((n_layers, n_heads, ccap), -1, np.int32)
+    local_cnt = np.zeros((n_layers, n_heads, nt), np.int32)
+    local_ptr = np.zeros((n_layers, n_heads, nt + 1), np.int32)
+    local_idx = np.full((n_layers, n_heads, max(lcap, 1)), -1, np.int32)
+    for l in lay:
+        for h in range(n_heads):
+            # ---- pass 1: count -------------------------------------------------------
+            ca_bits = [read_bits(ca_vec(l, h, d), ca_vector_bits(off[d + 1] - off[d], tile, gran)) for d in range(n_docs)]
+            ca_cnt = [int(b.sum()) for b in ca_bits]
+            cnt = np.zeros(nt, np.int64)
+            for d in range(n_docs):
+                lv = la_vec(l, h, d)
+                for i in range(int(p[d])):
+                    c = 0
+                    for j in range(i + 1):
+                        c += la_tile_bit(lv, i, j)
+                    cnt[int(base[d]) + i] = c
+            for t in range(int(base[n_docs]), nt):      # query M-blocks: all causal N-blocks
+                cnt[t] = t + 1
+            # ---- offsets -------------------------------------------------------------
+            cp = np.zeros(n_docs + 1, np.int64)
+            for d in range(n_docs):
+                cp[d + 1] = cp[d] + ca_cnt[d]
+            lp = np.zeros(nt + 1, np.int64)
+            for t in range(nt):
+                lp[t + 1] = lp[t] + cnt[t]
+            # ---- pass 2: fill (CA then LA, global coordinates) --------------------------
+            for d in range(n_docs):
+                w = int(cp[d])
+                for b in np.nonzero(ca_bits[d])[0]:
+                    cross_idx[l, h, w] = (off[d] + int(b)) if gran == 1 else (int(base[d]) + int(b))
+                    w += 1
+                assert w == cp[d + 1]
+            for d in range(n_docs):
+                lv = la_vec(l, h, d)
+                for i in range(int(p[d])):
+                    t = int(base[d]) + i
+                    w = int(lp[t])
+                    for j in range(i + 1):
+                        if la_tile_bit(lv, i, j):
+                            local_idx[l, h, w] = int(base[d]) + j
+                            w += 1
+            for t in range(int(base[n_docs]), nt):
+                local_idx[l, h, int(lp[t]): int(lp[t + 1])] = np.arange(t + 1)
+            cross_ptr[l, h], local_cnt[l, h], local_ptr[l, h] = cp, cnt, lp
+    out = dict(tt)
+    out.update(cross_ptr=cross_ptr, cross_idx=cross_idx, local_cnt=local_cnt, local_ptr=local_ptr,
+               local_idx=local_idx, cross_cap=ccap, local_cap=lcap)
+    return out
+
+
+def paper_view(md: Dict[str, np.ndarray], layer: int, head: int, t: int) -> np.ndarray:
+    """sparse_n_indices for (head, M-block t) as the paper lays it out (L239-245): the CA entries
+    of all earlier documents, then the LA entries; a query M-block is all causal N-blocks."""
+    n_docs = len(md["P"]) - 1
+    d = int(md["tile_seg"][t])
+    lo, hi = int(md["local_ptr"][layer, head, t]), int(md["local_ptr"][layer, head, t + 1])
+    loc = md["local_idx"][layer, head, lo:hi]
+    if d == n_docs:
+        return loc.copy()
+    return np.concatenate([md["cross_idx"][layer, head, : int(md["cross_ptr"][layer, head, d])], loc])
+
+
+def metadata_to_mask_rows(md: Dict[str, np.ndarray], doc_offsets: Sequence[int], query_len: int, tile: int,
+                          gran: int, layer: int, head: int, rows: Sequence[int]) -> np.ndarray:
+    """Inverse of decode: rebuild the boolean mask rows from MD-v1 (round-trip pin)."""
+    off = [int(x) for x in doc_offsets]
+    n_docs = len(off) - 1
+    n = off[-1] + query_len
+    row0, nrows, seg, base = md["tile_row0"], md["tile_rows"], md["tile_seg"], md["tile_base"]
+    out = np.zeros((len(rows), n), bool)
+    for ri, q in enumerate(rows):
+        q = int(q)
+        d = segment_of(q, off)
+        seg_start = off[d] if d < n_docs else off[-1]
+        t = int(base[d]) + (q - seg_start) // tile
+        if d < n_docs:
+            for e in md["cross_idx"][layer, head, : int(md["cross_ptr"][layer, head, d])]:
+                e = int(e)
+                if gran == 1:
+                    out[ri, e] = True
+                else:
+                    out[ri, int(row0[e]): int(row0[e]) + int(nrows[e])] = True
+        lo, hi = int(md["local_ptr"][layer, head, t]), int(md["local_ptr"][layer, head, t + 1])
+        for e in md["local_idx"][layer, head, lo:hi]:
+            e = int(e)
+            c0, c1 = int(row0[e]), int(row0[e]) + int(nrows[e])
+            out[ri, c0: min(c1, q + 1)] = True
+    return out
+
+
+def marked_pairs(doc_offsets: Sequence[int], query_len: int, tile: int, gran: int,
+                 la_vecs: Sequence[np.ndarray], ca_vecs: Sequence[np.ndarray], block: int = 256) -> int:
+    """Number of True mask entries of one (layer, head) (A26: element level)."""
+    n = int(doc_offsets[-1]) + query_len
+    tot = 0
+    for r0 in range(0, n, block):
+        rows = list(range(r0, min(n, r0 + block)))
+        tot += int(expand_mask_rows(doc_offsets, query_len, tile, gran, la_vecs, ca_vecs, rows).sum())
+    return tot
+
+
+# ------------------------------------------------------------------------------------------
+# Convenience for callers holding a workload-like object (duck-typed; no import of the package)
+# ------------------------------------------------------------------------------------------
+
+def head_vectors(w, layer: int, head: int) -> Tuple[List[np.ndarray], List[np.ndarray]]:
+    n_docs = len(w.shape.doc_lens)
+    return ([w.la_vec(layer, head, d) for d in range(n_docs)], [w.ca_vec(layer, head, d) for d in range(n_docs)])

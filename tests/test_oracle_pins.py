@@ -1,0 +1,347 @@
+"""Pins for oracle/sift_oracle.py against what the paper and the mathematics fix (no GPU).
+
+Each test names the passage of /root/reference/PAPER.md (cited as PAPER.md:L<line>) it pins.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import sift_oracle as so
+from paper_2606_09441_b200 import workload as wl
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ---------------------------------------------------------------- bit order / sizes
+
+def test_la_enumeration_order_L203():
+    # PAPER.md:L203 prints the order (0,0),(1,0),(1,1),(2,0)...
+    printed = [(0, 0), (1, 0), (1, 1), (2, 0)]
+    assert [so.la_bit_index(i, j) for (i, j) in printed] == [0, 1, 2, 3]
+    # row-major over the whole lower triangle is a bijection onto 0..P(P+1)/2-1
+    p = 7
+    seen = [so.la_bit_index(i, j) for i in range(p) for j in range(i + 1)]
+    assert seen == list(range(so.la_vector_bits(p)))
+
+
+def test_la_msb_first_hand_bytes_L203():
+    # P=3, diagonal tiles only: bits (0,0)=1,(1,0)=0,(1,1)=1,(2,0)=0,(2,1)=0,(2,2)=1 -> 1010 01xx, MSB first
+    vec = np.array([0xA4], np.uint8)
+    got = [[so.la_tile_bit(vec, i, j) for j in range(i + 1)] for i in range(3)]
+    assert got == [[1], [0, 1], [0, 0, 1]]
+    # P=8 all ones: 36 bits -> FF FF FF FF F0 (padded to the byte boundary, L203)
+    vec = np.array([0xFF, 0xFF, 0xFF, 0xFF, 0xF0], np.uint8)
+    assert all(so.la_tile_bit(vec, i, j) == 1 for i in range(8) for j in range(i + 1))
+    assert so.la_vector_bytes(8) == 5
+    # first bit of the stream is the MSB of byte 0
+    assert so.get_bit(np.array([0x80], np.uint8), 0) == 1 and so.get_bit(np.array([0x01], np.uint8), 7) == 1
+    assert so.get_bit(np.array([0x00, 0x40], np.uint8), 9) == 1
+
+
+def test_size_example_L213():
+    # "assuming P ~ 8 pages per document, the LA bit vector stores 36 bits and the CA bit vector stores 8 bits"
+    assert so.la_vector_bits(8) == 36
+    assert so.ca_vector_bits(1024, 128, 128) == 8
+    for p in range(1, 40):
+        assert so.la_vector_bytes(p) == math.ceil(p * (p + 1) / 16)
+        assert so.ca_vector_bytes(p * 128, 128, 128) == math.ceil(p / 8)
+    assert so.pages(2000, 128) == 16 and so.pages(2048, 128) == 16 and so.pages(2049, 128) == 17
+
+
+def _fmt(nbytes, unit):
+    return nbytes / 1024.0 if unit == "KB" else nbytes / (1024.0 * 1024.0)
+
+
+def test_table1_all_cells_L311():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "table1.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 9
+    for model, layers, heads, ctx, printed, unit in rows:
+        n_docs = int(ctx) // 1024
+        nbytes = so.sift_storage_bits(int(layers), int(heads), n_docs, 8) / 8.0
+        val = _fmt(nbytes, unit)
+        digits = 1 if "." in printed else 0
+        # the table prints truncated-or-rounded values; accept either
+        assert (round(val, digits) == float(printed)) or (math.floor(val * 10 ** digits) / 10 ** digits == float(printed)), \
+            (model, ctx, val, printed)
+
+
+def test_table1_ratios_and_breakeven_L307():
+    # KV bytes per token = layers * kv_heads * head_dim * 2 (K,V) * 2 B
+    kv = {"llama": 32 * 8 * 128 * 4, "qwen": 94 * 4 * 128 * 4, "minimax": 62 * 8 * 128 * 4}
+    sift_per_doc = {"llama": 32 * 32 * 44 / 8, "qwen": 94 * 64 * 44 / 8, "minimax": 62 * 48 * 44 / 8}
+    printed = {"llama": 23831, "qwen": 5958, "minimax": 15888}
+    for m in kv:
+        ratio = kv[m] * 1024 / sift_per_doc[m]
+        assert int(ratio) == printed[m] or round(ratio) == printed[m], (m, ratio)
+    # L307: sizes become equal at 33.6M tokens per doc (Llama 8B): P(P+1)/2 + P bits * 32*32 = 131072 B * 128 P
+    p = 2 * 131072 * 8 * 128 // (32 * 32)  # ~ solve P/2 * heads*layers = 8*kv*T
+    assert abs(p * 128 / 1e6 - 33.6) < 0.1
+    lhs = so.sift_storage_bits(32, 32, 1, p) / 8
+    rhs = kv["llama"] * p * 128
+    assert abs(lhs / rhs - 1.0) < 1e-3
+
+
+# ---------------------------------------------------------------- mask invariants
+
+def _vecs(w, layer=0, head=0):
+    return so.head_vectors(w, layer, head)
+
+
+def _mask(w, layer=0, head=0, rows=None):
+    sh = w.shape
+    la, ca = _vecs(w, layer, head)
+    rows = list(range(sh.n_tokens)) if rows is None else rows
+    return so.expand_mask_rows(sh.doc_offsets, sh.query_len, sh.tile, sh.cross_gran, la, ca, rows)
+
+
+@pytest.mark.parametrize("gran", [1, 32])
+def test_all_ones_is_dense_causal(gran):
+    # north_star; PAPER.md:L201-209 by construction
+    w = wl.custom("ones", doc_lens=(100, 64, 33), query_len=17, tile=32, cross_gran=gran, p_loc=1.1, p_cross=1.1)
+    n = w.shape.n_tokens
+    m = _mask(w)
+    assert np.array_equal(m, np.tril(np.ones((n, n), bool)))
+
+
+def test_cross_cleared_is_block_diagonal_plus_query():
+    # PAPER.md:L103 Fig 4a pattern; L147-149
+    w = wl.custom("nocross", doc_lens=(100, 64, 33), query_len=17, tile=32, p_loc=0.5, p_cross=-1.0,
+                  garbage_padding=True)
+    sh = w.shape
+    off = sh.doc_offsets
+    m = _mask(w)
+    for d in range(sh.n_docs):
+        blk = m[off[d]:off[d + 1]]
+        assert not blk[:, :off[d]].any() and not blk[:, off[d + 1]:].any()
+        assert np.array_equal(np.diag(blk[:, off[d]:off[d + 1]]), np.ones(off[d + 1] - off[d], bool))  # diag tiles set
+    qrows = m[off[-1]:]
+    n = sh.n_tokens
+    assert np.array_equal(qrows, np.tril(np.ones((n, n), bool))[off[-1]:])
+
+
+def test_mask_brute_force_definition():
+    # independent per-element restatement of SURVEY 8(c) Part 1 with explicit bit arithmetic
+    w = wl.custom("bf", n_q_heads=2, doc_lens=(70, 129, 40), query_len=9, tile=32, p_loc=0.4, p_cross=0.3, seed=5)
+    sh = w.shape
+    off = [int(x) for x in sh.doc_offsets]
+    for head in range(2):
+        la, ca = _vecs(w, 0, head)
+        m = _mask(w, 0, head)
+        n = sh.n_tokens
+        for q in range(0, n, 3):
+            for k in range(n):
+                if k > q:
+                    exp = False
+                elif q >= off[-1]:
+                    exp = True
+                else:
+                    d = max(i for i in range(sh.n_docs) if off[i] <= q)
+                    if k >= off[d]:
+                        i, j = (q - off[d]) // 32, (k - off[d]) // 32
+                        nbit = i * (i + 1) // 2 + j
+                        exp = bool(la[d][nbit // 8] & (0x80 >> (nbit % 8)))
+                    else:
+                        dp = max(i for i in range(sh.n_docs) if off[i] <= k)
+                        c = k - off[dp]
+                        exp = bool(ca[dp][c // 8] & (0x80 >> (c % 8)))
+                assert m[q, k] == exp, (q, k)
+
+
+def test_padding_bits_ignored_A6():
+    a = wl.custom("pad", doc_lens=(70, 45), query_len=5, tile=32, seed=3, garbage_padding=True)
+    b = wl.custom("pad", doc_lens=(70, 45), query_len=5, tile=32, seed=3, garbage_padding=False)
+    assert not np.array_equal(a.ca_blob, b.ca_blob) or not np.array_equal(a.la_blob, b.la_blob)
+    assert np.array_equal(_mask(a), _mask(b))
+
+
+def test_doc0_ignores_ca_and_query_ignores_both():
+    w = wl.custom("q", doc_lens=(64, 64), query_len=16, tile=32, p_loc=0.3, p_cross=0.5, seed=11)
+    m1 = _mask(w)
+    w2 = wl.custom("q", doc_lens=(64, 64), query_len=16, tile=32, p_loc=0.9, p_cross=0.1, seed=12)
+    m2 = _mask(w2)
+    assert np.array_equal(m1[128:], m2[128:])          # query rows: dense causal regardless of vectors
+    assert not m1[:64, 64:].any()
+
+
+def test_reorder_translates_local_blocks_L159():
+    w = wl.custom("ro", doc_lens=(96, 64, 40), query_len=8, tile=32, p_loc=0.4, p_cross=0.3, seed=21)
+    perm = [2, 0, 1]
+    w2 = w.reorder(perm)
+    m, m2 = _mask(w), _mask(w2)
+    off, off2 = w.shape.doc_offsets, w2.shape.doc_offsets
+    for p2, p1 in enumerate(perm):
+        a = m[off[p1]:off[p1 + 1], off[p1]:off[p1 + 1]]
+        b = m2[off2[p2]:off2[p2 + 1], off2[p2]:off2[p2 + 1]]
+        assert np.array_equal(a, b)
+    # cross columns of a doc are the same key set wherever it stands (seen from the last doc)
+    last_row_new = off2[3] - 1      # a row of doc at position 2 (old doc 1)
+    last_row_old_doc2_cols = m2[last_row_new, off2[0]:off2[1]]   # keys of old doc 2 seen from old doc 1
+    assert np.array_equal(last_row_old_doc2_cols, so.read_bits(w.ca_vec(0, 0, 2), 40))
+
+
+# ---------------------------------------------------------------- attention numerics
+
+def _attn(w, head, rows, dtype=torch.float64, layer=0):
+    sh = w.shape
+    q, k, v = w.qkv(layer)
+    la, ca = _vecs(w, layer, head)
+    return so.sift_attention_rows(q, k, v, head, sh.doc_offsets, sh.query_len, sh.tile, sh.cross_gran,
+                                  la, ca, rows, dtype=dtype), (q, k, v)
+
+
+def test_attention_brute_force_fp64_tiny():
+    w = wl.custom("bfa", n_q_heads=4, n_kv_heads=2, head_dim=16, doc_lens=(24, 19), query_len=6, tile=8,
+                  p_loc=0.4, p_cross=0.3, seed=7)
+    sh = w.shape
+    n = sh.n_tokens
+    for head in (0, 3):
+        (o, lse), (q, k, v) = _attn(w, head, list(range(n)))
+        m = _mask(w, 0, head)
+        kvh = head // 2                                  # A8 contiguous GQA groups
+        qn, kn, vn = q[:, head].double().numpy(), k[:, kvh].double().numpy(), v[:, kvh].double().numpy()
+        for r in range(n):
+            allowed = [int(x) for x in np.nonzero(m[r])[0]]
+            ob, lb = so.brute_force_row(qn[r], kn, vn, allowed, 1.0 / math.sqrt(16))
+            assert np.allclose(o[r].numpy(), ob, atol=1e-12)
+            assert abs(float(lse[r]) - lb) < 1e-12
+
+
+def test_all_ones_equals_torch_sdpa_causal():
+    # library special case: dense causal attention
+    w = wl.custom("sdpa", n_q_heads=2, n_kv_heads=1, head_dim=32, doc_lens=(40, 33), query_len=11, tile=16,
+                  p_loc=1.1, p_cross=1.1, seed=9)
+    n = w.shape.n_tokens
+    (o, lse), (q, k, v) = _attn(w, 1, list(range(n)), dtype=torch.float32)
+    ref = torch.nn.functional.scaled_dot_product_attention(
+        q[:, 1].float()[None, None], k[:, 0].float()[None, None], v[:, 0].float()[None, None], is_causal=True)[0, 0]
+    assert torch.allclose(o, ref, atol=2e-6)
+    od, lsed = so.dense_causal_rows(q, k, v, 1, list(range(n)), dtype=torch.float32)
+    assert torch.allclose(o, od, atol=1e-6) and torch.allclose(lse, lsed, atol=1e-6)
+
+
+def test_doc0_rows_equal_standalone_doc0_and_prefix_stability():
+    w = wl.custom("pre", n_q_heads=2, head_dim=16, doc_lens=(48, 40, 24), query_len=8, tile=16, seed=13)
+    (o, lse), (q, k, v) = _attn(w, 0, list(range(w.shape.n_tokens)))
+    # a prompt holding only doc 0 (+ query) gives the same doc-0 rows: appending docs leaves earlier rows unchanged
+    w0 = wl.custom("pre", n_q_heads=2, head_dim=16, doc_lens=(48,), query_len=8, tile=16, seed=13)
+    assert np.array_equal(w0.la_vec(0, 0, 0), w.la_vec(0, 0, 0))
+    (o0, lse0), _ = _attn(w0, 0, list(range(48)))
+    assert torch.allclose(o[:48], o0, atol=1e-13) and torch.allclose(lse[:48], lse0, atol=1e-13)
+
+
+def test_lse_merge_identity_and_weights_sum_to_one():
+    w = wl.custom("lse", n_q_heads=1, head_dim=16, doc_lens=(32, 32), query_len=4, tile=16, p_cross=0.5, seed=17)
+    sh = w.shape
+    q, k, v = w.qkv(0)
+    rows = list(range(32, 64))
+    m = _mask(w, rows=rows)
+    sc = 0.25
+    o, lse = so.attention_rows(q[rows, 0], k[:, 0], v[:, 0], m, sc, torch.float64)
+    mc, ml = m.copy(), m.copy()
+    mc[:, 32:] = False
+    ml[:, :32] = False
+    oc, lc = so.attention_rows(q[rows, 0], k[:, 0], v[:, 0], mc, sc, torch.float64)
+    ol, ll = so.attention_rows(q[rows, 0], k[:, 0], v[:, 0], ml, sc, torch.float64)
+    assert torch.allclose(lse, torch.logaddexp(lc, ll), atol=1e-12)
+    wc, wl_ = torch.exp(lc - lse), torch.exp(ll - lse)
+    assert torch.allclose(wc + wl_, torch.ones_like(wc), atol=1e-12)
+    assert torch.allclose(o, wc[:, None] * oc + wl_[:, None] * ol, atol=1e-12)
+    # V = ones -> O = ones (softmax weights sum to 1)
+    o1, _ = so.attention_rows(q[rows, 0], k[:, 0], torch.ones_like(v[:, 0]), m, sc, torch.float64)
+    assert torch.allclose(o1, torch.ones_like(o1), atol=1e-12)
+
+
+def test_empty_row_convention_A13():
+    w = wl.custom("empty", n_q_heads=1, head_dim=16, doc_lens=(32,), query_len=4, tile=16, p_loc=-1.0,
+                  p_cross=-1.0, diag_set=False, garbage_padding=False)
+    (o, lse), _ = _attn(w, 0, [0, 5, 31, 33])
+    assert torch.all(o[:3] == 0) and torch.all(torch.isinf(lse[:3])) and torch.all(lse[:3] < 0)
+    assert torch.isfinite(lse[3])
+
+
+# ---------------------------------------------------------------- metadata (MD-v1)
+
+def _md(w, **kw):
+    sh = w.shape
+    return so.decode_metadata(sh.doc_offsets, sh.query_len, sh.tile, sh.cross_gran, sh.n_layers, sh.n_q_heads,
+                              w.la_vec, w.ca_vec, **kw)
+
+
+@pytest.mark.parametrize("gran", [1, 16])
+def test_metadata_round_trip_reproduces_mask(gran):
+    w = wl.custom("rt", n_layers=2, n_q_heads=3, n_kv_heads=1, doc_lens=(70, 33, 64, 17), query_len=21, tile=16,
+                  cross_gran=gran, p_loc=0.35, p_cross=0.3, seed=23)
+    sh = w.shape
+    md = _md(w)
+    rows = list(range(sh.n_tokens))
+    for l in range(2):
+        for h in range(3):
+            la, ca = so.head_vectors(w, l, h)
+            m = so.expand_mask_rows(sh.doc_offsets, sh.query_len, sh.tile, gran, la, ca, rows)
+            m2 = so.metadata_to_mask_rows(md, sh.doc_offsets, sh.query_len, sh.tile, gran, l, h, rows)
+            assert np.array_equal(m, m2)
+
+
+def test_metadata_structure_L243_L245():
+    w = wl.custom("st", n_q_heads=2, doc_lens=(100, 64, 50), query_len=40, tile=32, p_loc=0.4, p_cross=0.25, seed=29)
+    sh = w.shape
+    md = _md(w)
+    off = sh.doc_offsets
+    nt, base = md["NT"], md["tile_base"]
+    assert list(md["P"]) == [4, 2, 2, 2] and nt == 10
+    for h in range(2):
+        cp, lp, cnt = md["cross_ptr"][0, h], md["local_ptr"][0, h], md["local_cnt"][0, h]
+        assert cp[0] == 0 and np.all(np.diff(cp) >= 0)
+        for d in range(3):                               # counts = number of valid set bits
+            assert cp[d + 1] - cp[d] == so.read_bits(w.ca_vec(0, h, d), sh.doc_lens[d]).sum()
+            seg = md["cross_idx"][0, h, cp[d]:cp[d + 1]]
+            assert np.all(np.diff(seg) > 0) and (len(seg) == 0 or (seg[0] >= off[d] and seg[-1] < off[d + 1]))
+        assert np.array_equal(np.diff(lp), cnt) and lp[0] == 0
+        for t in range(nt):
+            lst = md["local_idx"][0, h, lp[t]:lp[t + 1]]
+            assert np.all(np.diff(lst) > 0)
+            if t >= base[3]:                             # query M-block: all causal N-blocks (L243)
+                assert cnt[t] == t + 1 and np.array_equal(lst, np.arange(t + 1))
+            else:
+                d = md["tile_seg"][t]
+                assert np.all(lst >= base[d]) and np.all(lst <= t) and lst[-1] == t   # diagonal set
+        # paper-faithful list: CA entries then LA entries (L245)
+        t = int(base[2]) + 1
+        pv = so.paper_view(md, 0, h, t)
+        assert np.array_equal(pv[:cp[2]], md["cross_idx"][0, h, :cp[2]])
+        assert np.array_equal(pv[cp[2]:], md["local_idx"][0, h, lp[t]:lp[t + 1]])
+
+
+def test_metadata_hand_example():
+    # one doc of 3 tiles with LA = 0xA4 (diag only), second doc 2 tiles all ones; CA doc0 = 0b10010000 over 5 keys... G=1
+    sh = wl.PromptShape(1, 1, 1, 16, (12, 8), 4, tile=4, cross_gran=1)
+    la = [np.array([0xA4], np.uint8), np.array([0xE0], np.uint8)]
+    ca = [np.array([0x90, 0x10], np.uint8), np.array([0xFF], np.uint8)]
+    md = so.decode_metadata(sh.doc_offsets, 4, 4, 1, 1, 1, lambda l, h, d: la[d], lambda l, h, d: ca[d])
+    assert list(md["cross_ptr"][0, 0]) == [0, 3, 11]
+    assert list(md["cross_idx"][0, 0, :11]) == [0, 3, 11, 12, 13, 14, 15, 16, 17, 18, 19]
+    assert list(md["local_cnt"][0, 0]) == [1, 1, 1, 1, 2, 6]
+    assert list(md["local_idx"][0, 0, :12]) == [0, 1, 2, 3, 3, 4, 0, 1, 2, 3, 4, 5]
+
+
+def test_metadata_local_lists_invariant_under_reorder():
+    w = wl.custom("ro2", doc_lens=(96, 64, 40), query_len=8, tile=32, p_loc=0.4, p_cross=0.3, seed=31)
+    perm = [1, 2, 0]
+    w2 = w.reorder(perm)
+    a, b = _md(w), _md(w2)
+    for p2, p1 in enumerate(perm):
+        for i in range(int(a["P"][p1])):
+            t1, t2 = int(a["tile_base"][p1]) + i, int(b["tile_base"][p2]) + i
+            l1 = a["local_idx"][0, 0, a["local_ptr"][0, 0, t1]:a["local_ptr"][0, 0, t1 + 1]] - a["tile_base"][p1]
+            l2 = b["local_idx"][0, 0, b["local_ptr"][0, 0, t2]:b["local_ptr"][0, 0, t2 + 1]] - b["tile_base"][p2]
+            assert np.array_equal(l1, l2)
+
+
+def test_marked_pairs_counts():
+    w = wl.custom("mp", doc_lens=(50, 30), query_len=10, tile=16, p_loc=1.1, p_cross=1.1)
+    la, ca = so.head_vectors(w, 0, 0)
+    n = 90
+    assert so.marked_pairs(w.shape.doc_offsets, 10, 16, 1, la, ca) == n * (n + 1) // 2
