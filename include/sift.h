@@ -1,0 +1,118 @@
+/* sift.h -- C ABI of the B200-native SIFT hot path (arxiv/paper_2606_09441).
+ *
+ * Two operations, as the paper's implementation section states them:
+ *   sift_decode_metadata    PAPER.md:L237-247 (sec 5.1)  bit vectors -> packed int32 index lists
+ *   sift_prefill_attention  PAPER.md:L249-255 (sec 5.2)  block-sparse causal prefill attention driven by those lists
+ * plus a dense causal comparator from the same build ("Full Recompute").
+ *
+ * Conventions
+ *   - "dev" pointers are device memory owned by the caller; "HOST" pointers are host memory read during the
+ *     call and not retained.  The library never allocates or frees device memory, never synchronises the
+ *     stream and never reads device memory on the host.  All work is enqueued on `stream` (a cudaStream_t
+ *     passed as void*; NULL = the legacy default stream).
+ *   - Every call returns 0 (SIFT_OK) or a negative sift_status; on error nothing is enqueued.
+ *     sift_last_error() returns a thread-local, NUL-terminated description of the last failure.
+ *   - Prompt layout (Fig 6): n_docs documents concatenated, then the user query.
+ *     doc_offsets[0] = 0 < doc_offsets[1] < ... < doc_offsets[n_docs]; N = doc_offsets[n_docs] + query_len rows.
+ *   - Tiles are document-relative (reading A2): tile (d,i) covers rows doc_offsets[d] + i*tile ...;
+ *     the user query is segment n_docs.  Global tile id = tile_base[d] + i.
+ *   - Bit vectors: per (layer, q_head, document).  LA: lower triangle of the P x P tile
+ *     grid, row-major (0,0),(1,0),(1,1),(2,0).., MSB-first, ceil(P(P+1)/16) bytes, P = ceil(len/tile).
+ *     CA: one bit per group of `cross_gran` key tokens, MSB-first, ceil(ceil(len/cross_gran)/8) bytes.
+ *     Bits after the last valid bit of a vector are ignored.  One blob per document laid out
+ *     [layer][q_head][bytes]; la_doc_off[p] / ca_doc_off[p] = byte offset (from la_base / ca_base) of the blob
+ *     of the document at prompt position p.  The allocations must extend at least 4 bytes past the last vector
+ *     (the decoder reads aligned 32-bit words).
+ *   - GQA: q-head h uses kv-head h / (n_q_heads / n_kv_heads).
+ */
+#ifndef SIFT_H_
+#define SIFT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SIFT_MAX_DOCS 512
+
+typedef enum {
+  SIFT_OK = 0,
+  SIFT_ERR_INVALID_ARG = -1, /* NULL pointer, non-increasing offsets, misaligned tensor, ... */
+  SIFT_ERR_UNSUPPORTED = -2, /* head_dim not in {64,128}, tile not in {64,128}, cross_gran != 1, n_docs > SIFT_MAX_DOCS */
+  SIFT_ERR_WORKSPACE = -3,   /* metadata buffer too small */
+  SIFT_ERR_CUDA = -4         /* launch / driver error */
+} sift_status;
+
+typedef struct {
+  uint32_t struct_size; /* = sizeof(sift_shape) */
+  int32_t n_layers, n_q_heads, n_kv_heads, head_dim;
+  int32_t n_docs, query_len;
+  int32_t tile;       /* T: 64 or 128 (M-block = N-block = T) */
+  int32_t cross_gran; /* G: 1 = one CA bit per key token (BASELINE.json configs) */
+  const int32_t* doc_offsets; /* HOST, n_docs + 1 entries */
+} sift_shape;
+
+/* Byte offsets (from the start of the metadata buffer) of the arrays of container "MD-v1".
+ * All arrays are int32.  Canonical arrays (compared bit-exactly with the oracle):
+ *   tile_base [n_docs+2]           first global tile id of each segment; tile_base[n_docs+1] = NT
+ *   tile_seg/tile_row0/tile_rows [NT]
+ *   cross_ptr [L][Hq][n_docs+1]    cross_ptr[d] = number of marked keys in documents 0..d-1
+ *   cross_idx [L][Hq][cross_cap]   ascending global key rows; rows of document d attend entries [0, cross_ptr[d])
+ *   local_cnt [L][Hq][NT], local_ptr [L][Hq][NT+1], local_idx [L][Hq][local_cap]
+ *                                  per M-block: ascending global tile ids of marked LA tiles; query M-block t: 0..t
+ * Private arrays (scheduler): sched [L][n_items], counters [L][2]. */
+typedef struct {
+  uint32_t struct_size;
+  int32_t n_tiles;   /* NT */
+  int32_t cross_cap; /* per (layer, head) stride of cross_idx, multiple of 128 */
+  int32_t local_cap; /* per (layer, head) stride of local_idx */
+  int32_t n_mblocks; /* scheduler M-blocks per head */
+  int32_t n_items;   /* work items per layer = n_q_heads * n_mblocks */
+  size_t tile_base, tile_seg, tile_row0, tile_rows;
+  size_t cross_ptr, cross_idx, local_cnt, local_ptr, local_idx;
+  size_t mblock_tile0, sched, counters;
+  size_t total_bytes;
+} sift_md_layout;
+
+const char* sift_version(void);
+const char* sift_last_error(void);
+
+/* Size / layout of the metadata buffer for a shape.  Pure host arithmetic. */
+int sift_metadata_size(const sift_shape* shape, size_t* bytes);
+int sift_metadata_layout(const sift_shape* shape, sift_md_layout* out);
+
+/* PAPER.md:L237-247.  Pass 1 counts marked bits per (layer, head, M-block / document), an exclusive scan turns
+ * counts into offsets, pass 2 compacts the set bits into index lists in global coordinates.  All layers and heads
+ * in one call.  metadata: dev, 16-byte aligned, >= sift_metadata_size() bytes, fully overwritten. */
+int sift_decode_metadata(const sift_shape* shape,
+                         const uint8_t* la_base /*dev*/, const int64_t* la_doc_off /*HOST, n_docs*/,
+                         const uint8_t* ca_base /*dev*/, const int64_t* ca_doc_off /*HOST, n_docs*/,
+                         void* metadata /*dev, out*/, size_t metadata_bytes, void* stream);
+
+/* PAPER.md:L249-255.  One layer per call.  Q [N][n_q_heads][head_dim], K,V [N][n_kv_heads][head_dim], bf16, dev;
+ * row strides in elements (head stride = head_dim); bases and row strides 16-byte aligned.
+ * O [N][n_q_heads][head_dim] bf16 dev (out); lse [n_q_heads][N] fp32 dev (out, may be NULL): natural-log
+ * log-sum-exp of the scaled logits.  A row with no allowed key gets O = 0, lse = -inf.
+ * softmax_scale <= 0 selects 1/sqrt(head_dim).  fp32 accumulation; P is rounded to bf16 before P*V.
+ * Calls that use the same (metadata, layer) must be stream-ordered (they share a work counter). */
+int sift_prefill_attention(const sift_shape* shape, int32_t layer,
+                           const void* Q, const void* K, const void* V,
+                           int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
+                           const void* metadata /*dev, from sift_decode_metadata*/,
+                           void* O, int64_t o_row_stride, float* lse, float softmax_scale, void* stream);
+
+/* Dense causal attention over n_tokens rows with the same kernel body (no metadata). */
+int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
+                                const void* Q, const void* K, const void* V,
+                                int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
+                                void* O, int64_t o_row_stride, float* lse, float softmax_scale, void* stream);
+
+/* Number of kernels the library has launched in this process (bench.py's gpu_launches). */
+int64_t sift_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SIFT_H_ */

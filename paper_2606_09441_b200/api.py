@@ -1,0 +1,201 @@
+"""ctypes binding of libsift_b200.so (include/sift.h).  Argument marshalling only: every step of the hot
+path runs in the library's CUDA kernels.  There is no CPU fallback: a missing library raises."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Dict, Optional, Tuple
+
+import numpy as np
+import torch
+
+from .build import LIB
+
+SIFT_OK = 0
+EXPORTS = ("sift_version", "sift_last_error", "sift_metadata_size", "sift_metadata_layout",
+           "sift_decode_metadata", "sift_prefill_attention", "sift_dense_causal_attention", "sift_launch_count")
+
+
+class SiftShape(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_layers", C.c_int32), ("n_q_heads", C.c_int32),
+                ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32), ("n_docs", C.c_int32),
+                ("query_len", C.c_int32), ("tile", C.c_int32), ("cross_gran", C.c_int32),
+                ("doc_offsets", C.POINTER(C.c_int32))]
+
+
+class SiftMdLayout(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_tiles", C.c_int32), ("cross_cap", C.c_int32),
+                ("local_cap", C.c_int32), ("n_mblocks", C.c_int32), ("n_items", C.c_int32)] + \
+               [(n, C.c_size_t) for n in ("tile_base", "tile_seg", "tile_row0", "tile_rows", "cross_ptr", "cross_idx",
+                                          "local_cnt", "local_ptr", "local_idx", "mblock_tile0", "sched", "counters",
+                                          "total_bytes")]
+
+
+class SiftError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB):
+            raise SiftError(f"{LIB} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                            "(there is no CPU fallback)")
+        L = C.CDLL(LIB)
+        L.sift_version.restype = C.c_char_p
+        L.sift_last_error.restype = C.c_char_p
+        L.sift_launch_count.restype = C.c_int64
+        L.sift_metadata_size.argtypes = [C.POINTER(SiftShape), C.POINTER(C.c_size_t)]
+        L.sift_metadata_layout.argtypes = [C.POINTER(SiftShape), C.POINTER(SiftMdLayout)]
+        L.sift_decode_metadata.argtypes = [C.POINTER(SiftShape), C.c_void_p, C.POINTER(C.c_int64), C.c_void_p,
+                                           C.POINTER(C.c_int64), C.c_void_p, C.c_size_t, C.c_void_p]
+        L.sift_prefill_attention.argtypes = [C.POINTER(SiftShape), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                             C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_int64,
+                                             C.c_void_p, C.c_float, C.c_void_p]
+        L.sift_dense_causal_attention.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
+                                                  C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_int64,
+                                                  C.c_void_p, C.c_float, C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != SIFT_OK:
+        raise SiftError(f"{what} failed ({rc}): {lib().sift_last_error().decode()}")
+
+
+def sift_version() -> str:
+    return lib().sift_version().decode()
+
+
+def sift_launch_count() -> int:
+    return int(lib().sift_launch_count())
+
+
+@dataclass
+class Shape:
+    """Python mirror of sift_shape; keeps the host offset array alive."""
+    n_layers: int
+    n_q_heads: int
+    n_kv_heads: int
+    head_dim: int
+    doc_offsets: np.ndarray
+    query_len: int
+    tile: int
+    cross_gran: int = 1
+
+    def __post_init__(self):
+        self.doc_offsets = np.ascontiguousarray(self.doc_offsets, dtype=np.int32)
+        self._c = SiftShape(C.sizeof(SiftShape), self.n_layers, self.n_q_heads, self.n_kv_heads, self.head_dim,
+                            len(self.doc_offsets) - 1, self.query_len, self.tile, self.cross_gran,
+                            self.doc_offsets.ctypes.data_as(C.POINTER(C.c_int32)))
+
+    @classmethod
+    def from_prompt(cls, ps) -> "Shape":
+        return cls(ps.n_layers, ps.n_q_heads, ps.n_kv_heads, ps.head_dim, ps.doc_offsets, ps.query_len, ps.tile,
+                   ps.cross_gran)
+
+    @property
+    def n_tokens(self) -> int:
+        return int(self.doc_offsets[-1]) + self.query_len
+
+    @property
+    def c(self) -> SiftShape:
+        return self._c
+
+
+def sift_metadata_layout(shape: Shape) -> SiftMdLayout:
+    lay = SiftMdLayout()
+    _check(lib().sift_metadata_layout(C.byref(shape.c), C.byref(lay)), "sift_metadata_layout")
+    return lay
+
+
+def sift_metadata_size(shape: Shape) -> int:
+    n = C.c_size_t(0)
+    _check(lib().sift_metadata_size(C.byref(shape.c), C.byref(n)), "sift_metadata_size")
+    return int(n.value)
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _i64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int64)
+
+
+def sift_decode_metadata(shape: Shape, la_base: torch.Tensor, la_doc_off, ca_base: torch.Tensor, ca_doc_off,
+                         metadata: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """la_base/ca_base: uint8 CUDA tensors; returns the metadata buffer (uint8 CUDA tensor)."""
+    assert la_base.is_cuda and ca_base.is_cuda and la_base.dtype == torch.uint8 and ca_base.dtype == torch.uint8
+    if metadata is None:
+        metadata = torch.empty(sift_metadata_size(shape), dtype=torch.uint8, device=la_base.device)
+    lo, co = _i64(la_doc_off), _i64(ca_doc_off)
+    rc = lib().sift_decode_metadata(C.byref(shape.c), la_base.data_ptr(), lo.ctypes.data_as(C.POINTER(C.c_int64)),
+                                    ca_base.data_ptr(), co.ctypes.data_as(C.POINTER(C.c_int64)),
+                                    metadata.data_ptr(), metadata.numel(), _stream(stream))
+    _check(rc, "sift_decode_metadata")
+    return metadata
+
+
+def _check_qkv(q, k, v):
+    for t in (q, k, v):
+        assert t.is_cuda and t.dtype == torch.bfloat16 and t.dim() == 3 and t.stride(2) == 1 and t.stride(1) == t.shape[2]
+
+
+def sift_prefill_attention(shape: Shape, layer: int, q: torch.Tensor, k: torch.Tensor, v: torch.Tensor,
+                           metadata: torch.Tensor, out: Optional[torch.Tensor] = None,
+                           lse: Optional[torch.Tensor] = None, softmax_scale: float = 0.0, return_lse: bool = True,
+                           stream=None) -> Tuple[torch.Tensor, Optional[torch.Tensor]]:
+    _check_qkv(q, k, v)
+    if out is None:
+        out = torch.empty_like(q)
+    if lse is None and return_lse:
+        lse = torch.empty((q.shape[1], q.shape[0]), dtype=torch.float32, device=q.device)
+    rc = lib().sift_prefill_attention(C.byref(shape.c), layer, q.data_ptr(), k.data_ptr(), v.data_ptr(),
+                                      q.stride(0), k.stride(0), v.stride(0), metadata.data_ptr(), out.data_ptr(),
+                                      out.stride(0), lse.data_ptr() if lse is not None else None,
+                                      float(softmax_scale), _stream(stream))
+    _check(rc, "sift_prefill_attention")
+    return out, lse
+
+
+def sift_dense_causal_attention(q: torch.Tensor, k: torch.Tensor, v: torch.Tensor, out: Optional[torch.Tensor] = None,
+                                lse: Optional[torch.Tensor] = None, softmax_scale: float = 0.0,
+                                return_lse: bool = True, stream=None) -> Tuple[torch.Tensor, Optional[torch.Tensor]]:
+    _check_qkv(q, k, v)
+    if out is None:
+        out = torch.empty_like(q)
+    if lse is None and return_lse:
+        lse = torch.empty((q.shape[1], q.shape[0]), dtype=torch.float32, device=q.device)
+    rc = lib().sift_dense_causal_attention(q.shape[0], q.shape[1], k.shape[1], q.shape[2], q.data_ptr(), k.data_ptr(),
+                                           v.data_ptr(), q.stride(0), k.stride(0), v.stride(0), out.data_ptr(),
+                                           out.stride(0), lse.data_ptr() if lse is not None else None,
+                                           float(softmax_scale), _stream(stream))
+    _check(rc, "sift_dense_causal_attention")
+    return out, lse
+
+
+def metadata_views(shape: Shape, metadata: torch.Tensor) -> Dict[str, torch.Tensor]:
+    """int32 views of the MD-v1 arrays inside the buffer (no copies)."""
+    lay = sift_metadata_layout(shape)
+    m32 = metadata.view(torch.int32)
+    L, H, D, NT = shape.n_layers, shape.n_q_heads, len(shape.doc_offsets) - 1, lay.n_tiles
+
+    def v(off, *dims):
+        n = int(np.prod(dims))
+        return m32[off // 4: off // 4 + n].view(*dims)
+    return {
+        "tile_base": v(lay.tile_base, D + 2), "tile_seg": v(lay.tile_seg, NT), "tile_row0": v(lay.tile_row0, NT),
+        "tile_rows": v(lay.tile_rows, NT), "cross_ptr": v(lay.cross_ptr, L, H, D + 1),
+        "cross_idx": v(lay.cross_idx, L, H, lay.cross_cap), "local_cnt": v(lay.local_cnt, L, H, NT),
+        "local_ptr": v(lay.local_ptr, L, H, NT + 1), "local_idx": v(lay.local_idx, L, H, lay.local_cap),
+        "mblock_tile0": v(lay.mblock_tile0, lay.n_mblocks + 1), "sched": v(lay.sched, L, lay.n_items),
+        "counters": v(lay.counters, L, 2),
+    }

@@ -1,0 +1,647 @@
+// SIFT block-sparse causal prefill attention for sm_100a (sec 5.2; mask per L147-149, L201-209).
+//
+// Paper design (FlashAttention-3 on H200: TMA + wgmma, the N-block index read from sparse_n_indices[i]) is prior art.
+// This kernel keeps the idea "an index list drives which K/V tile the copy engine fetches" and is otherwise built for
+// Blackwell:
+//   * persistent CTAs (one per SM) pull (q-head, M-block) work items, longest first, through an atomic counter;
+//   * an M-block is kNQ query tiles of 128 TMEM lanes of the same document and head: they share the head's cross
+//     list, so every gathered K/V tile in shared memory feeds kNQ accumulators;
+//   * warp roles: warp 0 = producer (TMA; `tile::gather4` for the row-granular cross keys, tiled boxes for local
+//     tiles and the dense query rows), warp 1 = tcgen05.mma issuer, warp 2 = TMEM allocator, warps 4.. = one softmax
+//     warpgroup per query tile (one row per thread, S read with tcgen05.ld, P written back to TMEM as bf16 and used
+//     as the A operand of the P*V MMA, lazy rescale of the TMEM-resident O accumulator);
+//   * S = Q K^T and O += P V are tcgen05.mma.kind::f16 (bf16 in, fp32 accumulate in TMEM).
+// Work decomposition of one DOC item (document d >= 0, head h):
+//   cross phase  groups of 128 entries of cross_idx[h][0 .. cross_ptr[h][d])        (a6 in DESIGN.md)
+//   local phase  union of the tiles' local lists; the diagonal tile is causally masked  (a7)
+// and of a DENSE item (user-query rows, or the dense comparator): key blocks 0,128,.. up to the last row (a8).
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <math.h>
+#include <string.h>
+
+#include "sift_common.h"
+#include "sm100_ptx.cuh"
+
+namespace sift {
+using namespace ptx;
+
+constexpr int kNQ = SIFT_Q_TILES_PER_ITEM;  // query tiles per work item
+constexpr int kBM = 128;                    // rows of one query tile = TMEM lanes
+constexpr int kBN = 128;                    // keys per step
+constexpr int kNumThreads = 128 + 128 * kNQ;
+constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 with a stale max
+constexpr uint32_t kTmemCols = 512;
+
+struct AttnParams {
+  // metadata (null in dense mode)
+  const int32_t *tile_seg, *tile_row0, *tile_rows, *mblock_tile0;
+  const int32_t *cross_ptr, *cross_idx, *local_cnt, *local_ptr, *local_idx;  // already offset to the layer
+  const int32_t* sched;                                                      // already offset to the layer
+  int32_t* counters;                                                         // [2]: next item, finished CTAs
+  int32_t n_items, n_docs, n_tiles, cross_cap, local_cap, n_mblocks;
+  int32_t dense;  // 1: every M-block is a DENSE item over n_tokens rows
+  int32_t n_tokens, n_q_heads, n_kv_heads, tile;
+  __nv_bfloat16* o;
+  int64_t o_row_stride;
+  float* lse;  // [Hq][N] or null
+  float scale_log2;
+};
+
+template <int HD>
+struct Smem {
+  static constexpr int kHalves = HD / 64;
+  static constexpr int kTileBytes = kBN * HD * 2;          // one K or V tile / one Q tile
+  static constexpr int kKStages = (kNQ == 1) ? 3 : (HD == 128 ? 3 : 4);
+  static constexpr int kVStages = (kNQ == 1) ? 3 : (HD == 128 ? 2 : 4);
+  static constexpr int kQOff = 0;
+  static constexpr int kKOff = kQOff + kNQ * kTileBytes;
+  static constexpr int kVOff = kKOff + kKStages * kTileBytes;
+  static constexpr int kBarOff = kVOff + kVStages * kTileBytes;
+  // barrier slots (8 B each)
+  static constexpr int bQFull = 0, bQEmpty = 1;
+  static constexpr int bKFull = 2, bKEmpty = bKFull + kKStages;
+  static constexpr int bVFull = bKEmpty + kKStages, bVEmpty = bVFull + kVStages;
+  static constexpr int bSFull = bVEmpty + kVStages, bPFull = bSFull + kNQ, bODone = bPFull + kNQ;
+  static constexpr int bItemFull = bODone + kNQ, bItemEmpty = bItemFull + 2;
+  static constexpr int kNumBars = bItemEmpty + 2;
+  static constexpr int kInfoOff = kBarOff + ((kNumBars * 8 + 15) / 16) * 16;
+  // info words: [0] tmem base, [1..2] item ring, [4 .. 4+kKStages) per-K-stage step info
+  static constexpr int kBytes = kInfoOff + 64 + 1024;      // + slack for the manual 1024-byte alignment
+};
+
+// One work item as every role sees it.
+struct Item {
+  int h, kvh;
+  int is_dense;            // DENSE (query rows / comparator) or DOC
+  int row0[kNQ], rows[kNQ];  // global first row and valid rows of each query tile (rows <= 0: tile absent)
+  int tile_id[kNQ];
+  int cp;                  // DOC: number of cross entries of its document
+  int lptr[kNQ], lcnt[kNQ];  // DOC: local list of each tile
+};
+
+__device__ __forceinline__ Item load_item(const AttnParams& p, int code) {
+  Item it;
+  const int h = code >> 20, mb = code & 0xFFFFF;
+  it.h = h;
+  it.kvh = h / (p.n_q_heads / p.n_kv_heads);
+  it.cp = 0;
+  if (p.dense) {
+    it.is_dense = 1;
+#pragma unroll
+    for (int q = 0; q < kNQ; ++q) {
+      it.row0[q] = (mb * kNQ + q) * kBM;
+      it.rows[q] = min(kBM, p.n_tokens - it.row0[q]);
+      it.tile_id[q] = 0; it.lptr[q] = 0; it.lcnt[q] = 0;
+    }
+    return it;
+  }
+  const int t0 = p.mblock_tile0[mb];
+  const int nt = min(kNQ, p.mblock_tile0[mb + 1] - t0);
+  const int seg = p.tile_seg[t0];
+  it.is_dense = (seg == p.n_docs);
+  const int64_t lh = h;  // pointers are already offset to the layer
+  if (!it.is_dense) it.cp = p.cross_ptr[lh * (p.n_docs + 1) + seg];
+#pragma unroll
+  for (int q = 0; q < kNQ; ++q) {
+    if (q < nt) {
+      it.tile_id[q] = t0 + q;
+      it.row0[q] = p.tile_row0[t0 + q];
+      it.rows[q] = p.tile_rows[t0 + q];
+      it.lptr[q] = p.local_ptr[lh * (p.n_tiles + 1) + t0 + q];
+      it.lcnt[q] = p.local_cnt[lh * p.n_tiles + t0 + q];
+    } else {
+      it.tile_id[q] = -1; it.row0[q] = 0; it.rows[q] = 0; it.lptr[q] = 0; it.lcnt[q] = 0;
+    }
+  }
+  return it;
+}
+
+// number of key blocks a DENSE tile attends: keys 0 .. row0+rows-1
+__device__ __forceinline__ int dense_steps(int row0, int rows) { return rows > 0 ? (row0 + rows + kBN - 1) / kBN : 0; }
+
+
+// ------------------------------------------------------------------------------------------------
+// descriptors
+// ------------------------------------------------------------------------------------------------
+// Q / K tile in smem: HD/64 halves of [128 rows x 128 B], 128-byte swizzle (what TMA writes).  K-chunk k (16 bf16):
+template <int HD>
+__device__ __forceinline__ uint64_t kmajor_desc(uint32_t tile_addr, int k) {
+  return umma_desc_sw128(tile_addr + (k >> 2) * (kBN * 128) + (k & 3) * 32, 16, 1024);
+}
+// V tile, same smem image, used MN-major (N = head dim contiguous): K-chunk k = 16 key rows = 2 KB further
+template <int HD>
+__device__ __forceinline__ uint64_t v_desc(uint32_t tile_addr, int k) {
+  return umma_desc_sw128(tile_addr + k * 2048, kBN * 128, 1024);
+}
+
+template <int HD>
+__global__ void __launch_bounds__(kNumThreads, 1)
+sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                      const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_kg,
+                      const __grid_constant__ CUtensorMap tm_vg, const AttnParams p) {
+  using S = Smem<HD>;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t sbase = (raw + 1023u) & ~1023u;
+  uint8_t* sgen = smem_raw + (sbase - raw);
+  const uint32_t bar0 = sbase + S::kBarOff;
+  auto bar = [&](int i) -> uint32_t { return bar0 + i * 8; };
+  volatile int32_t* info = reinterpret_cast<volatile int32_t*>(sgen + S::kInfoOff);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  constexpr uint32_t idesc_qk = umma_idesc_bf16(kBM, kBN, 0, 0);
+  constexpr uint32_t idesc_pv = umma_idesc_bf16(kBM, HD, 0, 1);
+
+  if (warp == 0 && lane == 0) {
+    mbar_init(bar(S::bQFull), 1);
+    mbar_init(bar(S::bQEmpty), 1);
+    for (int i = 0; i < S::kKStages; ++i) { mbar_init(bar(S::bKFull + i), 1); mbar_init(bar(S::bKEmpty + i), 1); }
+    for (int i = 0; i < S::kVStages; ++i) { mbar_init(bar(S::bVFull + i), 1); mbar_init(bar(S::bVEmpty + i), 1); }
+    for (int q = 0; q < kNQ; ++q) {
+      mbar_init(bar(S::bSFull + q), 1);
+      mbar_init(bar(S::bPFull + q), 128);
+      mbar_init(bar(S::bODone + q), 1);
+    }
+    for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 1 + 128 * kNQ); }
+    fence_barrier_init();
+    prefetch_tensormap(&tm_q); prefetch_tensormap(&tm_k); prefetch_tensormap(&tm_v);
+    prefetch_tensormap(&tm_kg); prefetch_tensormap(&tm_vg);
+  }
+  if (warp == 2) {
+    tmem_alloc(smem_u32(const_cast<int32_t*>(&info[0])), kTmemCols);
+    tmem_relinquish();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = static_cast<uint32_t>(info[0]);
+
+  if (warp == 0) {
+    // ======================================= producer =======================================
+    uint32_t kst = 0, kph = 0, vst = 0, vph = 0;
+    const uint32_t q_smem = sbase + S::kQOff, k_smem = sbase + S::kKOff, v_smem = sbase + S::kVOff;
+    for (int it_n = 0;; ++it_n) {
+      const int slot = it_n & 1;
+      mbar_wait(bar(S::bItemEmpty + slot), ((it_n >> 1) & 1) ^ 1, 100);
+      int code = -1;
+      if (lane == 0) {
+        const int idx = atomicAdd(&p.counters[0], 1);
+        if (idx < p.n_items) {
+          code = p.dense ? (((idx % p.n_q_heads) << 20) | (p.n_mblocks - 1 - idx / p.n_q_heads)) : p.sched[idx];
+        } else {
+          const int f = atomicAdd(&p.counters[1], 1);
+          if (f == (int)gridDim.x - 1) { atomicExch(&p.counters[0], 0); atomicExch(&p.counters[1], 0); }
+        }
+        info[1 + slot] = code;
+        mbar_arrive(bar(S::bItemFull + slot));
+      }
+      code = __shfl_sync(0xffffffffu, code, 0);
+      if (code < 0) break;
+      const Item it = load_item(p, code);
+      // ---- Q tiles
+      mbar_wait(bar(S::bQEmpty), (it_n & 1) ^ 1, 101);
+      if (lane == 0) {
+        mbar_arrive_expect_tx(bar(S::bQFull), kNQ * S::kTileBytes);
+#pragma unroll
+        for (int q = 0; q < kNQ; ++q)
+#pragma unroll
+          for (int hf = 0; hf < S::kHalves; ++hf)
+            tma_load_2d(q_smem + q * S::kTileBytes + hf * (kBM * 128), &tm_q, bar(S::bQFull), it.h * HD + hf * 64,
+                        it.row0[q]);
+      }
+      __syncwarp();
+      // ---- K/V tiles, one step at a time
+      auto emit = [&](bool gather, int src, int act, bool last) {
+        // src: gather -> index of the first cross entry of the group; tiled -> first key row
+        int4 r = make_int4(0, 0, 0, 0);
+        if (gather) r = *reinterpret_cast<const int4*>(p.cross_idx + (int64_t)it.h * p.cross_cap + src + lane * 4);
+        mbar_wait(bar(S::bKEmpty + kst), kph ^ 1, 102);
+        if (lane == 0) {
+          info[4 + kst] = act | (last ? 4 : 0);
+          mbar_arrive_expect_tx(bar(S::bKFull + kst), S::kTileBytes);
+        }
+        __syncwarp();
+        const uint32_t kdst = k_smem + kst * S::kTileBytes;
+        if (gather) {
+#pragma unroll
+          for (int hf = 0; hf < S::kHalves; ++hf)
+            tma_gather4(kdst + hf * (kBN * 128) + lane * 512, &tm_kg, bar(S::bKFull + kst), it.kvh * HD + hf * 64, r.x,
+                        r.y, r.z, r.w);
+        } else if (lane == 0) {
+#pragma unroll
+          for (int hf = 0; hf < S::kHalves; ++hf)
+            tma_load_2d(kdst + hf * (kBN * 128), &tm_k, bar(S::bKFull + kst), it.kvh * HD + hf * 64, src);
+        }
+        if (++kst == S::kKStages) { kst = 0; kph ^= 1; }
+        mbar_wait(bar(S::bVEmpty + vst), vph ^ 1, 103);
+        if (lane == 0) mbar_arrive_expect_tx(bar(S::bVFull + vst), S::kTileBytes);
+        __syncwarp();
+        const uint32_t vdst = v_smem + vst * S::kTileBytes;
+        if (gather) {
+#pragma unroll
+          for (int hf = 0; hf < S::kHalves; ++hf)
+            tma_gather4(vdst + hf * (kBN * 128) + lane * 512, &tm_vg, bar(S::bVFull + vst), it.kvh * HD + hf * 64, r.x,
+                        r.y, r.z, r.w);
+        } else if (lane == 0) {
+#pragma unroll
+          for (int hf = 0; hf < S::kHalves; ++hf)
+            tma_load_2d(vdst + hf * (kBN * 128), &tm_v, bar(S::bVFull + vst), it.kvh * HD + hf * 64, src);
+        }
+        if (++vst == S::kVStages) { vst = 0; vph ^= 1; }
+      };
+      if (it.is_dense) {
+        int n[kNQ], total = 0;
+#pragma unroll
+        for (int q = 0; q < kNQ; ++q) { n[q] = dense_steps(it.row0[q], it.rows[q]); total = max(total, n[q]); }
+        for (int j = 0; j < total; ++j) {
+          int act = 0;
+#pragma unroll
+          for (int q = 0; q < kNQ; ++q) act |= (j < n[q]) << q;
+          emit(false, j * kBN, act, j == total - 1);
+        }
+      } else {
+        int present = 0, nloc = 0;
+#pragma unroll
+        for (int q = 0; q < kNQ; ++q) { present |= (it.rows[q] > 0) << q; nloc += it.lcnt[q]; }
+        const int ngroups = (it.cp + kBN - 1) / kBN;
+        for (int g = 0; g < ngroups; ++g) emit(true, g * kBN, present, g == ngroups - 1 && nloc == 0);
+        const int32_t* lidx = p.local_idx + (int64_t)it.h * p.local_cap;
+        int pos[kNQ];
+#pragma unroll
+        for (int q = 0; q < kNQ; ++q) pos[q] = 0;
+        while (true) {
+          int cur[kNQ], t = 0x7fffffff;
+#pragma unroll
+          for (int q = 0; q < kNQ; ++q) {
+            cur[q] = pos[q] < it.lcnt[q] ? lidx[it.lptr[q] + pos[q]] : 0x7fffffff;
+            t = min(t, cur[q]);
+          }
+          if (t == 0x7fffffff) break;
+          int act = 0, remaining = 0;
+#pragma unroll
+          for (int q = 0; q < kNQ; ++q) {
+            if (cur[q] == t) { act |= 1 << q; ++pos[q]; }
+            remaining += it.lcnt[q] - pos[q];
+          }
+          emit(false, p.tile_row0[t], act, remaining == 0);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ======================================= MMA issuer =======================================
+    if (lane == 0) {
+      uint32_t kst = 0, kph = 0, vst = 0, vph = 0, pph[kNQ];
+#pragma unroll
+      for (int q = 0; q < kNQ; ++q) pph[q] = 0;
+      const uint32_t q_smem = sbase + S::kQOff, k_smem = sbase + S::kKOff, v_smem = sbase + S::kVOff;
+      for (int it_n = 0;; ++it_n) {
+        const int slot = it_n & 1;
+        mbar_wait(bar(S::bItemFull + slot), (it_n >> 1) & 1, 200);
+        const int code = info[1 + slot];
+        mbar_arrive(bar(S::bItemEmpty + slot));
+        if (code < 0) break;
+        const Item it = load_item(p, code);
+        bool has_steps = it.is_dense || it.cp > 0;
+#pragma unroll
+        for (int q = 0; q < kNQ; ++q) has_steps = has_steps || it.lcnt[q] > 0;
+        mbar_wait(bar(S::bQFull), it_n & 1, 201);
+        if (!has_steps) { mbar_arrive(bar(S::bQEmpty)); continue; }
+        tc_fence_after();
+        int pending = 0;
+        uint32_t accum[kNQ];
+#pragma unroll
+        for (int q = 0; q < kNQ; ++q) accum[q] = 0;
+        auto flush_pv = [&](int q, bool& v_waited) {
+          mbar_wait(bar(S::bPFull + q), pph[q], 202);
+          pph[q] ^= 1;
+          if (!v_waited) { mbar_wait(bar(S::bVFull + vst), vph, 203); v_waited = true; }
+          tc_fence_after();
+          const uint32_t vt = v_smem + vst * S::kTileBytes;
+#pragma unroll
+          for (int k = 0; k < kBN / 16; ++k)
+            umma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + k * 8, v_desc<HD>(vt, k), idesc_pv, accum[q] | (k > 0));
+          accum[q] = 1;
+          umma_commit(bar(S::bODone + q));
+        };
+        bool last = false;
+        while (!last) {
+          mbar_wait(bar(S::bKFull + kst), kph, 204);
+          const int inf = info[4 + kst];
+          const int act = inf & 3;
+          last = (inf & 4) != 0;
+          tc_fence_after();
+          bool v_waited = false;
+          const uint32_t kt = k_smem + kst * S::kTileBytes;
+#pragma unroll
+          for (int q = 0; q < kNQ; ++q) {
+            if (pending & (1 << q)) flush_pv(q, v_waited);
+            if (act & (1 << q)) {
+#pragma unroll
+              for (int k = 0; k < HD / 16; ++k)
+                umma_ss(tmem_base + q * 128, kmajor_desc<HD>(q_smem + q * S::kTileBytes, k), kmajor_desc<HD>(kt, k), idesc_qk, k > 0);
+              umma_commit(bar(S::bSFull + q));
+            }
+          }
+          if (pending) {
+            umma_commit(bar(S::bVEmpty + vst));
+            if (++vst == S::kVStages) { vst = 0; vph ^= 1; }
+          }
+          umma_commit(bar(S::bKEmpty + kst));
+          if (++kst == S::kKStages) { kst = 0; kph ^= 1; }
+          pending = act;
+        }
+        umma_commit(bar(S::bQEmpty));   // every Q K^T of this item has been issued
+        bool v_waited = false;
+#pragma unroll
+        for (int q = 0; q < kNQ; ++q)
+          if (pending & (1 << q)) flush_pv(q, v_waited);
+        umma_commit(bar(S::bVEmpty + vst));
+        if (++vst == S::kVStages) { vst = 0; vph ^= 1; }
+      }
+    }
+  } else if (warp >= 4) {
+    // ======================================= softmax warpgroups =======================================
+    const int q = (warp - 4) >> 2;
+    const int r = threadIdx.x - 128 - q * 128;             // row inside the query tile = TMEM lane
+    const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
+    const uint32_t s_addr = tmem_base + lane_addr + q * 128;
+    const uint32_t o_addr = tmem_base + lane_addr + 256 + q * 128;
+    const float sl = p.scale_log2;
+    uint32_t sph = 0;
+    uint32_t pv_cnt = 0;
+    for (int it_n = 0;; ++it_n) {
+      const int slot = it_n & 1;
+      mbar_wait(bar(S::bItemFull + slot), (it_n >> 1) & 1, 300);
+      const int code = info[1 + slot];
+      mbar_arrive(bar(S::bItemEmpty + slot));
+      if (code < 0) break;
+      const Item it = load_item(p, code);
+      if (it.rows[q] <= 0) continue;
+      const int ngroups = it.is_dense ? 0 : (it.cp + kBN - 1) / kBN;
+      const int nsteps = it.is_dense ? dense_steps(it.row0[q], it.rows[q]) : ngroups + it.lcnt[q];
+      bool last_is_diag = false;
+      if (!it.is_dense && it.lcnt[q] > 0)
+        last_is_diag = p.local_idx[(int64_t)it.h * p.local_cap + it.lptr[q] + it.lcnt[q] - 1] == it.tile_id[q];
+      float m = -INFINITY, l = 0.f;
+      for (int e = 0; e < nsteps; ++e) {
+        int n_valid = kBN, kdelta = 0;
+        bool causal = false;
+        if (it.is_dense) {
+          kdelta = e * kBN - it.row0[q];
+          causal = kdelta + kBN - 1 > 0;
+        } else if (e < ngroups) {
+          n_valid = min(kBN, it.cp - e * kBN);
+        } else {
+          n_valid = min(kBN, p.tile);
+          causal = last_is_diag && (e == nsteps - 1);
+        }
+        mbar_wait(bar(S::bSFull + q), sph, 301);
+        sph ^= 1;
+        tc_fence_after();
+        float s[kBN];
+#pragma unroll
+        for (int c = 0; c < kBN / 32; ++c) tmem_ld32(s_addr + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
+        tmem_wait_ld();
+        if (causal || n_valid < kBN) {
+          const int lim = causal ? min(n_valid, r - kdelta + 1) : n_valid;   // columns [0, lim) are allowed
+#pragma unroll
+          for (int c = 0; c < kBN; ++c) s[c] = (c < lim) ? s[c] : -INFINITY;
+        }
+        float mx = s[0];
+#pragma unroll
+        for (int c = 1; c < kBN; ++c) mx = fmaxf(mx, s[c]);
+        const float m_new = fmaxf(m, mx);
+        const bool need = (m_new - m) * sl > kRescaleThreshold;   // (-inf) - (-inf) = NaN -> false
+        if (__any_sync(0xffffffffu, need)) {
+          const float alpha = need ? ex2((m - m_new) * sl) : 1.f;
+          l *= alpha;
+          if (need) m = m_new;
+          if (e > 0) {
+            // O of this tile must hold every P*V issued so far before it is rescaled
+            mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 302);
+            tc_fence_after();
+#pragma unroll
+            for (int c = 0; c < HD / 32; ++c) {
+              uint32_t o[32];
+              tmem_ld32(o_addr + c * 32, o);
+              tmem_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+              tmem_st32(o_addr + c * 32, o);
+            }
+          }
+        }
+        const float neg_m = (m == -INFINITY) ? 0.f : -m * sl;
+        float sum = 0.f;
+#pragma unroll
+        for (int c = 0; c < kBN / 32; ++c) {
+          uint32_t pk[16];
+#pragma unroll
+          for (int i = 0; i < 16; ++i) {
+            const float p0 = ex2(fmaf(s[c * 32 + 2 * i], sl, neg_m));
+            const float p1 = ex2(fmaf(s[c * 32 + 2 * i + 1], sl, neg_m));
+            sum += p0 + p1;
+            pk[i] = pack_bf16x2(p0, p1);
+          }
+          // P (bf16) overwrites the first 64 columns of S: 16 packed columns per 32 keys
+          asm volatile(
+              "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+              ::"r"(s_addr + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
+                "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
+                "r"(pk[15]) : "memory");
+        }
+        l += sum;
+        tmem_wait_st();
+        tc_fence_before();
+        mbar_arrive(bar(S::bPFull + q));
+        ++pv_cnt;
+      }
+      // ---- epilogue: O / l -> bf16, LSE
+      const int64_t grow = (int64_t)it.row0[q] + r;
+      const bool row_ok = r < it.rows[q];
+      __nv_bfloat16* orow = p.o + grow * p.o_row_stride + (int64_t)it.h * HD;
+      if (nsteps > 0) {
+        mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 303);
+        tc_fence_after();
+        const float inv = l > 0.f ? 1.f / l : 0.f;
+#pragma unroll
+        for (int c = 0; c < HD / 32; ++c) {
+          uint32_t o[32];
+          tmem_ld32(o_addr + c * 32, o);
+          tmem_wait_ld();
+          if (row_ok) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              uint4 w;
+              w.x = pack_bf16x2(__uint_as_float(o[8 * i + 0]) * inv, __uint_as_float(o[8 * i + 1]) * inv);
+              w.y = pack_bf16x2(__uint_as_float(o[8 * i + 2]) * inv, __uint_as_float(o[8 * i + 3]) * inv);
+              w.z = pack_bf16x2(__uint_as_float(o[8 * i + 4]) * inv, __uint_as_float(o[8 * i + 5]) * inv);
+              w.w = pack_bf16x2(__uint_as_float(o[8 * i + 6]) * inv, __uint_as_float(o[8 * i + 7]) * inv);
+              *reinterpret_cast<uint4*>(orow + c * 32 + i * 8) = w;
+            }
+          }
+        }
+        tc_fence_before();
+      } else if (row_ok) {
+#pragma unroll
+        for (int i = 0; i < HD / 8; ++i) *reinterpret_cast<uint4*>(orow + i * 8) = make_uint4(0, 0, 0, 0);
+      }
+      if (row_ok && p.lse != nullptr)
+        p.lse[(int64_t)it.h * p.n_tokens + grow] = (l > 0.f) ? (m * sl + log2f(l)) * 0.6931471805599453f : -INFINITY;
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) tmem_dealloc(tmem_base, kTmemCols);
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (fn) return fn;
+  void* sym = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess ||
+      qres != cudaDriverEntryPointSuccess)
+    return nullptr;
+  fn = reinterpret_cast<EncodeTiledFn>(sym);
+  return fn;
+}
+
+// 2-D bf16 tensor [rows][cols] with row stride `row_stride` elements; box = 64 columns x box_rows, 128B swizzle
+static int make_map(CUtensorMap* m, const void* base, int64_t rows, int64_t cols, int64_t row_stride, int box_rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return set_error(SIFT_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+  cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t gstr[1] = {(cuuint64_t)row_stride * 2};
+  cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstr, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return set_error(SIFT_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  return SIFT_OK;
+}
+
+static int g_num_sms = 0;
+__device__ int32_t g_dense_counters[2] = {0, 0};
+
+static int check_tensor(const void* ptr, int64_t stride, const char* name) {
+  if (!ptr) return set_error(SIFT_ERR_INVALID_ARG, "%s is NULL", name);
+  if (((uintptr_t)ptr & 15) != 0 || (stride * 2) % 16 != 0)
+    return set_error(SIFT_ERR_INVALID_ARG, "%s base / row stride not 16-byte aligned", name);
+  return SIFT_OK;
+}
+
+template <int HD>
+static int launch_attention(AttnParams& p, const void* Q, const void* K, const void* V, int64_t qs, int64_t ks, int64_t vs,
+                            cudaStream_t st) {
+  CUtensorMap tq, tk, tv, tkg, tvg;
+  int rc;
+  const int64_t n = p.n_tokens;
+  if ((rc = make_map(&tq, Q, n, (int64_t)p.n_q_heads * HD, qs, kBM))) return rc;
+  if ((rc = make_map(&tk, K, n, (int64_t)p.n_kv_heads * HD, ks, kBN))) return rc;
+  if ((rc = make_map(&tv, V, n, (int64_t)p.n_kv_heads * HD, vs, kBN))) return rc;
+  if ((rc = make_map(&tkg, K, n, (int64_t)p.n_kv_heads * HD, ks, 1))) return rc;
+  if ((rc = make_map(&tvg, V, n, (int64_t)p.n_kv_heads * HD, vs, 1))) return rc;
+  if (g_num_sms == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (g_num_sms <= 0) g_num_sms = 148;
+  }
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(sift_attention_kernel<HD>, cudaFuncAttributeMaxDynamicSharedMemorySize, Smem<HD>::kBytes);
+    if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "cudaFuncSetAttribute(smem=%d): %s", Smem<HD>::kBytes, cudaGetErrorString(e));
+    attr_set = true;
+  }
+  const int grid = p.n_items < g_num_sms ? (p.n_items > 0 ? p.n_items : 1) : g_num_sms;
+  cudaGetLastError();
+  sift_attention_kernel<HD><<<grid, kNumThreads, Smem<HD>::kBytes, st>>>(tq, tk, tv, tkg, tvg, p);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "attention launch: %s", cudaGetErrorString(e));
+  count_launch(1);
+  return SIFT_OK;
+}
+
+}  // namespace sift
+
+using namespace sift;
+
+extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, const void* Q, const void* K, const void* V,
+                                      int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
+                                      const void* metadata, void* O, int64_t o_row_stride, float* lse,
+                                      float softmax_scale, void* stream) {
+  sift_md_layout lay;
+  int rc = compute_layout(shape, &lay);
+  if (rc) return rc;
+  if (layer < 0 || layer >= shape->n_layers) return set_error(SIFT_ERR_INVALID_ARG, "layer %d out of range", layer);
+  if (!metadata) return set_error(SIFT_ERR_INVALID_ARG, "metadata is NULL");
+  if ((rc = check_tensor(Q, q_row_stride, "Q")) || (rc = check_tensor(K, k_row_stride, "K")) ||
+      (rc = check_tensor(V, v_row_stride, "V")) || (rc = check_tensor(O, o_row_stride, "O")))
+    return rc;
+  const int Hq = shape->n_q_heads, D = shape->n_docs, HD = shape->head_dim;
+  if (q_row_stride < (int64_t)Hq * HD || o_row_stride < (int64_t)Hq * HD || k_row_stride < (int64_t)shape->n_kv_heads * HD ||
+      v_row_stride < (int64_t)shape->n_kv_heads * HD)
+    return set_error(SIFT_ERR_INVALID_ARG, "row stride smaller than heads*head_dim");
+  const char* b = static_cast<const char*>(metadata);
+  auto at = [&](size_t off) { return reinterpret_cast<const int32_t*>(b + off); };
+  AttnParams p;
+  memset(&p, 0, sizeof(p));
+  const int64_t lh0 = (int64_t)layer * Hq;
+  p.tile_seg = at(lay.tile_seg); p.tile_row0 = at(lay.tile_row0); p.tile_rows = at(lay.tile_rows);
+  p.mblock_tile0 = at(lay.mblock_tile0);
+  p.cross_ptr = at(lay.cross_ptr) + lh0 * (D + 1);
+  p.cross_idx = at(lay.cross_idx) + lh0 * lay.cross_cap;
+  p.local_cnt = at(lay.local_cnt) + lh0 * lay.n_tiles;
+  p.local_ptr = at(lay.local_ptr) + lh0 * (lay.n_tiles + 1);
+  p.local_idx = at(lay.local_idx) + lh0 * lay.local_cap;
+  p.sched = at(lay.sched) + (int64_t)layer * lay.n_items;
+  p.counters = const_cast<int32_t*>(at(lay.counters)) + layer * 2;
+  p.n_items = lay.n_items; p.n_docs = D; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap;
+  p.local_cap = lay.local_cap; p.n_mblocks = lay.n_mblocks;
+  p.dense = 0;
+  p.n_tokens = shape->doc_offsets[D] + shape->query_len;
+  p.n_q_heads = Hq; p.n_kv_heads = shape->n_kv_heads; p.tile = shape->tile;
+  p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
+  const float sc = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf((float)HD);
+  p.scale_log2 = sc * 1.4426950408889634f;
+  if (HD == 128) return launch_attention<128>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
+  return launch_attention<64>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
+}
+
+extern "C" int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
+                                           const void* Q, const void* K, const void* V, int64_t q_row_stride,
+                                           int64_t k_row_stride, int64_t v_row_stride, void* O, int64_t o_row_stride,
+                                           float* lse, float softmax_scale, void* stream) {
+  if (n_tokens < 1 || n_tokens > (1 << 20) || n_q_heads < 1 || n_q_heads > 255 || n_kv_heads < 1 || n_q_heads % n_kv_heads)
+    return set_error(SIFT_ERR_INVALID_ARG, "bad dimensions");
+  if (head_dim != 64 && head_dim != 128) return set_error(SIFT_ERR_UNSUPPORTED, "head_dim %d not in {64,128}", head_dim);
+  int rc;
+  if ((rc = check_tensor(Q, q_row_stride, "Q")) || (rc = check_tensor(K, k_row_stride, "K")) ||
+      (rc = check_tensor(V, v_row_stride, "V")) || (rc = check_tensor(O, o_row_stride, "O")))
+    return rc;
+  AttnParams p;
+  memset(&p, 0, sizeof(p));
+  p.dense = 1;
+  p.n_tokens = n_tokens; p.n_q_heads = n_q_heads; p.n_kv_heads = n_kv_heads; p.tile = 128;
+  p.n_mblocks = (n_tokens + kBM * kNQ - 1) / (kBM * kNQ);
+  p.n_items = p.n_mblocks * n_q_heads;
+  void* cptr = nullptr;
+  if (cudaGetSymbolAddress(&cptr, g_dense_counters) != cudaSuccess) return set_error(SIFT_ERR_CUDA, "no device symbol");
+  p.counters = static_cast<int32_t*>(cptr);
+  p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
+  const float sc = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf((float)head_dim);
+  p.scale_log2 = sc * 1.4426950408889634f;
+  if (head_dim == 128) return launch_attention<128>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
+  return launch_attention<64>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
+}

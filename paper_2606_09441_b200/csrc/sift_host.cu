@@ -1,0 +1,149 @@
+// Host side of the C ABI: validation, MD-v1 layout arithmetic, error reporting, sift_decode_metadata entry.
+#include <stdarg.h>
+#include <string.h>
+
+#include "sift_common.h"
+
+namespace sift {
+
+static thread_local char g_err[512] = "";
+static std::atomic<int64_t> g_launches{0};
+
+int set_error(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+int validate_shape(const sift_shape* s) {
+  if (!s) return set_error(SIFT_ERR_INVALID_ARG, "shape is NULL");
+  if (s->struct_size != sizeof(sift_shape))
+    return set_error(SIFT_ERR_INVALID_ARG, "shape.struct_size %u != %zu", s->struct_size, sizeof(sift_shape));
+  if (!s->doc_offsets) return set_error(SIFT_ERR_INVALID_ARG, "shape.doc_offsets is NULL");
+  if (s->n_layers < 1 || s->n_q_heads < 1 || s->n_kv_heads < 1 || s->n_docs < 0 || s->query_len < 0)
+    return set_error(SIFT_ERR_INVALID_ARG, "negative or zero dimension");
+  if (s->n_q_heads % s->n_kv_heads != 0)
+    return set_error(SIFT_ERR_INVALID_ARG, "n_q_heads %d not a multiple of n_kv_heads %d", s->n_q_heads, s->n_kv_heads);
+  if (s->n_q_heads > 255) return set_error(SIFT_ERR_UNSUPPORTED, "n_q_heads %d > 255", s->n_q_heads);
+  if (s->head_dim != 64 && s->head_dim != 128)
+    return set_error(SIFT_ERR_UNSUPPORTED, "head_dim %d not in {64,128}", s->head_dim);
+  if (s->tile != 64 && s->tile != 128) return set_error(SIFT_ERR_UNSUPPORTED, "tile %d not in {64,128}", s->tile);
+  if (s->cross_gran != 1)
+    return set_error(SIFT_ERR_UNSUPPORTED, "cross_gran %d: only 1 (per key token) is built", s->cross_gran);
+  if (s->n_docs > SIFT_MAX_DOCS) return set_error(SIFT_ERR_UNSUPPORTED, "n_docs %d > %d", s->n_docs, SIFT_MAX_DOCS);
+  if (s->doc_offsets[0] != 0) return set_error(SIFT_ERR_INVALID_ARG, "doc_offsets[0] != 0");
+  for (int d = 0; d < s->n_docs; ++d)
+    if (s->doc_offsets[d + 1] <= s->doc_offsets[d])
+      return set_error(SIFT_ERR_INVALID_ARG, "doc_offsets not strictly increasing at %d", d);
+  int64_t n = (int64_t)s->doc_offsets[s->n_docs] + s->query_len;
+  if (n < 1 || n > (1 << 20)) return set_error(SIFT_ERR_UNSUPPORTED, "prompt of %lld rows (1 .. 2^20 supported)", (long long)n);
+  return SIFT_OK;
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+int compute_layout(const sift_shape* s, sift_md_layout* out) {
+  int rc = validate_shape(s);
+  if (rc) return rc;
+  const int T = s->tile, D = s->n_docs, NQ = SIFT_Q_TILES_PER_ITEM;
+  int64_t nt = 0, lcap = 0, nmb = 0;
+  for (int d = 0; d < D; ++d) {
+    int64_t p = ceil_div_i(s->doc_offsets[d + 1] - s->doc_offsets[d], T);
+    nt += p;
+    lcap += p * (p + 1) / 2;
+    nmb += (p + NQ - 1) / NQ;
+  }
+  int64_t pq = ceil_div_i(s->query_len, T);
+  for (int64_t t = nt; t < nt + pq; ++t) lcap += t + 1;
+  nt += pq;
+  nmb += (pq + NQ - 1) / NQ;
+  int64_t ccap = (int64_t)ceil_div_i(ceil_div_i(s->doc_offsets[D], s->cross_gran), 128) * 128;
+  if (lcap >= (1ll << 31) || ccap >= (1ll << 31)) return set_error(SIFT_ERR_UNSUPPORTED, "index capacity >= 2^31");
+  if (lcap < 1) lcap = 1;
+  const int64_t LH = (int64_t)s->n_layers * s->n_q_heads;
+  memset(out, 0, sizeof(*out));
+  out->struct_size = sizeof(sift_md_layout);
+  out->n_tiles = (int32_t)nt;
+  out->cross_cap = (int32_t)ccap;
+  out->local_cap = (int32_t)lcap;
+  out->n_mblocks = (int32_t)nmb;
+  out->n_items = (int32_t)(nmb * s->n_q_heads);
+  size_t o = 0;
+  auto take = [&](int64_t n_int32) { size_t r = o; o = align_up(o + (size_t)n_int32 * 4, 128); return r; };
+  out->tile_base = take(D + 2);
+  out->tile_seg = take(nt);
+  out->tile_row0 = take(nt);
+  out->tile_rows = take(nt);
+  out->cross_ptr = take(LH * (D + 1));
+  out->cross_idx = take(LH * ccap);
+  out->local_cnt = take(LH * nt);
+  out->local_ptr = take(LH * (nt + 1));
+  out->local_idx = take(LH * lcap);
+  out->mblock_tile0 = take(nmb + 1);
+  out->sched = take((int64_t)s->n_layers * out->n_items);
+  out->counters = take((int64_t)s->n_layers * 2);
+  out->total_bytes = o;
+  return SIFT_OK;
+}
+
+}  // namespace sift
+
+using namespace sift;
+
+extern "C" {
+
+#define SIFT_STR2(x) #x
+#define SIFT_STR(x) SIFT_STR2(x)
+const char* sift_version(void) {
+  return "sift-b200 0.1.0 (sm_100a; MD-v1; q_tiles_per_item=" SIFT_STR(SIFT_Q_TILES_PER_ITEM) ")";
+}
+
+const char* sift_last_error(void) { return g_err; }
+
+int64_t sift_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+int sift_metadata_layout(const sift_shape* shape, sift_md_layout* out) {
+  if (!out) return set_error(SIFT_ERR_INVALID_ARG, "out is NULL");
+  return compute_layout(shape, out);
+}
+
+int sift_metadata_size(const sift_shape* shape, size_t* bytes) {
+  if (!bytes) return set_error(SIFT_ERR_INVALID_ARG, "bytes is NULL");
+  sift_md_layout lay;
+  int rc = compute_layout(shape, &lay);
+  if (rc) return rc;
+  *bytes = lay.total_bytes;
+  return SIFT_OK;
+}
+
+int sift_decode_metadata(const sift_shape* shape, const uint8_t* la_base, const int64_t* la_doc_off,
+                         const uint8_t* ca_base, const int64_t* ca_doc_off, void* metadata, size_t metadata_bytes,
+                         void* stream) {
+  sift_md_layout lay;
+  int rc = compute_layout(shape, &lay);
+  if (rc) return rc;
+  if (!metadata) return set_error(SIFT_ERR_INVALID_ARG, "metadata is NULL");
+  if (((uintptr_t)metadata & 15) != 0) return set_error(SIFT_ERR_INVALID_ARG, "metadata not 16-byte aligned");
+  if (metadata_bytes < lay.total_bytes)
+    return set_error(SIFT_ERR_WORKSPACE, "metadata buffer %zu < %zu bytes", metadata_bytes, lay.total_bytes);
+  if (shape->n_docs > 0 && (!la_base || !ca_base || !la_doc_off || !ca_doc_off))
+    return set_error(SIFT_ERR_INVALID_ARG, "bit-vector pointer is NULL");
+  static thread_local DocTable dt;
+  dt.n_docs = shape->n_docs;
+  dt.query_len = shape->query_len;
+  dt.tile = shape->tile;
+  dt.gran = shape->cross_gran;
+  for (int d = 0; d <= shape->n_docs; ++d) dt.off[d] = shape->doc_offsets[d];
+  for (int d = 0; d < shape->n_docs; ++d) {
+    if (la_doc_off[d] < 0 || ca_doc_off[d] < 0) return set_error(SIFT_ERR_INVALID_ARG, "negative blob offset at doc %d", d);
+    dt.la_off[d] = la_doc_off[d];
+    dt.ca_off[d] = ca_doc_off[d];
+  }
+  return launch_decode(shape, lay, dt, la_base, ca_base, metadata, (cudaStream_t)stream);
+}
+
+}  // extern "C"
