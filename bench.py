@@ -1,0 +1,339 @@
+#!/usr/bin/env python
+"""bench.py -- SIFT hot path on B200: metadata decode + block-sparse prefill attention for one layer.
+
+A "step" = sift_decode_metadata (all heads of the layer) + sift_prefill_attention over one synthetic RAG prompt.
+Default workload = BASELINE.json configs[2] ("32K context": 16 docs x 2000 + 256 query, 32/8 GQA heads, d=128), one of
+the two contexts the metric is quoted on; --with-64k (default on) also times configs[3] and reports it in "extra".
+Metric: effective TFLOP/s over marked pairs = 4*d*(true mask entries)/time.
+
+    python bench.py --gpus 1 --steps 20 --warmup 5
+    python -m torch.distributed.run --nproc-per-node N ... bench.py --gpus N   (weak scaling: one prompt per rank)
+    python bench.py --impl reference        (the CPU oracle, as it stands, on a bounded sample)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_09441_b200 import workload as wl  # noqa: E402
+
+METRIC = "effective TFLOP/s (marked pairs), sparse prefill attention + metadata decode, 1 layer"
+UNIT = "TFLOP/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        j = json.load(open(p))
+        return {"bf16": float(j["bf16_tflops"]), "bf16_sustained": float(j.get("bf16_tflops_sustained", j["bf16_tflops"])),
+                "hbm": float(j["hbm_gbs"]), "src": "measured"}
+    return {"bf16": 1590.0, "bf16_sustained": 1400.0, "hbm": 6650.0, "src": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+
+    def __init__(self, dev: int):
+        self.dev, self.rows, self.proc = dev, [], None
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.dev), f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(sm)}
+
+
+def dist_setup(n_gpus: int):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl" if torch.cuda.is_available() else "gloo")
+    return rank, world, local
+
+
+def barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def max_over_ranks(x: float, world: int) -> float:
+    if world == 1:
+        return x
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device="cuda" if torch.cuda.is_available() else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(x: float, world: int) -> float:
+    if world == 1:
+        return x
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device="cuda" if torch.cuda.is_available() else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+# --------------------------------------------------------------------------------------------- GPU arm
+
+class GpuCase:
+    """One prompt resident on the device + the calls of one step."""
+
+    def __init__(self, w, layer=0):
+        from paper_2606_09441_b200 import api, metrics
+        self.api, self.w, self.layer = api, w, layer
+        self.shape = api.Shape.from_prompt(w.shape)
+        self.la_h = torch.from_numpy(w.la_blob).pin_memory()
+        self.ca_h = torch.from_numpy(w.ca_blob).pin_memory()
+        q, k, v = w.qkv(layer)
+        self.q_h, self.k_h, self.v_h = q.pin_memory(), k.pin_memory(), v.pin_memory()
+        self.la, self.ca = self.la_h.cuda(), self.ca_h.cuda()
+        self.q, self.k, self.v = self.q_h.cuda(), self.k_h.cuda(), self.v_h.cuda()
+        self.md = torch.empty(api.sift_metadata_size(self.shape), dtype=torch.uint8, device="cuda")
+        self.o = torch.empty_like(self.q)
+        self.lse = torch.empty((q.shape[1], q.shape[0]), dtype=torch.float32, device="cuda")
+        self.o_h = torch.empty(self.o.shape, dtype=self.o.dtype).pin_memory()
+        self.decode()
+        torch.cuda.synchronize()
+        views = {k_: t.cpu().numpy() for k_, t in api.metadata_views(self.shape, self.md).items()}
+        self.pairs = int(metrics.marked_pairs_per_head(views, layer, w.shape.n_docs).sum())
+        self.flops = metrics.attention_flops(self.pairs, w.shape.head_dim)
+        self.dense_flops = metrics.attention_flops(metrics.dense_causal_pairs(w.shape.n_tokens) * w.shape.n_q_heads,
+                                                   w.shape.head_dim)
+        self.decode_bytes = metrics.decode_algorithmic_bytes(w.shape, api.sift_metadata_layout(self.shape), views)
+
+    def decode(self):
+        self.api.sift_decode_metadata(self.shape, self.la, self.w.la_doc_off, self.ca, self.w.ca_doc_off, self.md)
+
+    def attention(self):
+        self.api.sift_prefill_attention(self.shape, self.layer, self.q, self.k, self.v, self.md, self.o, self.lse)
+
+    def dense(self):
+        self.api.sift_dense_causal_attention(self.q, self.k, self.v, self.o, self.lse)
+
+    def step(self):
+        self.decode()
+        self.attention()
+
+    def e2e_step(self):
+        """Same step through the public API with HOST buffers: H2D of bit vectors and Q/K/V, D2H of O."""
+        self.la.copy_(self.la_h, non_blocking=True)
+        self.ca.copy_(self.ca_h, non_blocking=True)
+        self.q.copy_(self.q_h, non_blocking=True)
+        self.k.copy_(self.k_h, non_blocking=True)
+        self.v.copy_(self.v_h, non_blocking=True)
+        self.step()
+        self.o_h.copy_(self.o, non_blocking=True)
+
+    @property
+    def h2d_bytes(self):
+        return sum(t.numel() * t.element_size() for t in (self.la_h, self.ca_h, self.q_h, self.k_h, self.v_h))
+
+    @property
+    def d2h_bytes(self):
+        return self.o_h.numel() * self.o_h.element_size()
+
+
+def time_region(fn, steps):
+    """CUDA events on the current stream around `steps` calls; returns total ms."""
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(steps):
+        fn()
+    b.record()
+    b.synchronize()
+    return a.elapsed_time(b)
+
+
+def time_each(fn, steps):
+    """Per-call CUDA-event durations (ms)."""
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        a.record()
+        fn()
+        b.record()
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in ev]
+
+
+def cpu_oracle_sample(w, layer=0, budget_rows=384, heads=(0, 13), seed=0):
+    """The oracle as it stands on a bounded sample of the same workload: `budget_rows` sampled rows of two heads.
+    Returns (effective TFLOP/s over the marked pairs of those rows, seconds, cores, description)."""
+    from oracle import sift_oracle as so
+    sh = w.shape
+    q, k, v = w.qkv(layer)
+    rng = np.random.default_rng(seed)
+    rows = sorted(int(x) for x in rng.choice(sh.n_tokens, size=min(budget_rows, sh.n_tokens), replace=False))
+    heads = [h for h in heads if h < sh.n_q_heads]
+    pairs = 0
+    t0 = time.perf_counter()
+    for h in heads:
+        la, ca = so.head_vectors(w, layer, h)
+        so.sift_attention_rows(q, k, v, h, sh.doc_offsets, sh.query_len, sh.tile, sh.cross_gran, la, ca, rows)
+    dt = time.perf_counter() - t0
+    for h in heads:       # pair count outside the timed region
+        la, ca = so.head_vectors(w, layer, h)
+        pairs += int(so.expand_mask_rows(sh.doc_offsets, sh.query_len, sh.tile, sh.cross_gran, la, ca, rows).sum())
+    tf = 4 * sh.head_dim * pairs / dt / 1e12
+    return tf, dt, torch.get_num_threads(), f"{len(rows)} seeded rows x heads {heads} of {w.name} (mask expansion + fp32 masked softmax)"
+
+
+def run_ours(args):
+    rank, world, local = dist_setup(args.gpus)
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    from paper_2606_09441_b200 import api
+    peaks = load_peaks()
+    seed = wl.BASE_SEED + rank
+    w = wl.CONFIGS[args.config](seed) if args.config != "full-stack" else wl.config_full_stack(seed, 2)
+    case = GpuCase(w)
+    for _ in range(max(args.warmup, 3)):
+        case.step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    launches0 = api.sift_launch_count()
+    barrier(world)
+    torch.cuda.synchronize()
+    sampler.start()
+    ms_total = time_region(case.step, args.steps)
+    torch.cuda.synchronize()
+    barrier(world)
+    launches = api.sift_launch_count() - launches0
+    clocks = sampler.stop()
+    ms_step = max_over_ranks(ms_total / args.steps, world)
+    flops_all = sum_over_ranks(float(case.flops), world)
+    value = flops_all / (ms_step * 1e-3) / 1e12
+
+    # per-kernel timings (same stream, after the headline region)
+    att = time_each(case.attention, args.steps)
+    dec = time_each(case.decode, args.steps)
+    den = time_each(case.dense, max(3, args.steps // 4))
+    att_ms, dec_ms, den_ms = float(np.mean(att)), float(np.mean(dec)), float(np.mean(den))
+    achieved = case.flops / (att_ms * 1e-3) / 1e12
+
+    # end to end with host buffers
+    for _ in range(2):
+        case.e2e_step()
+    torch.cuda.synchronize()
+    barrier(world)
+    e2e_ms = max_over_ranks(time_region(case.e2e_step, max(3, args.steps // 4)) / max(3, args.steps // 4), world)
+    e2e_val = flops_all / (e2e_ms * 1e-3) / 1e12
+
+    extra = {"attention_ms": att_ms, "attention_ms_best": float(np.min(att)), "decode_us": dec_ms * 1e3,
+             "dense_causal_ms": den_ms, "dense_tflops": case.dense_flops / (den_ms * 1e-3) / 1e12,
+             "speedup_vs_dense": den_ms / att_ms, "marked_density": case.flops / case.dense_flops,
+             "decode_GBps": case.decode_bytes / (dec_ms * 1e-3) / 1e9, "decode_bytes": case.decode_bytes,
+             "frac_of_sustained_peak": achieved / peaks["bf16_sustained"], "n_tokens": w.shape.n_tokens}
+    if args.with_64k and args.config == "32k" and world == 1:
+        c4 = GpuCase(wl.config_64k_ragged(seed))
+        for _ in range(3):
+            c4.step()
+        a4 = float(np.mean(time_each(c4.attention, max(3, args.steps // 2))))
+        d4 = float(np.mean(time_each(c4.dense, 3)))
+        k4 = float(np.mean(time_each(c4.decode, max(3, args.steps // 2))))
+        extra["64k"] = {"n_tokens": c4.w.shape.n_tokens, "attention_ms": a4, "effective_tflops": c4.flops / (a4 * 1e-3) / 1e12,
+                        "dense_causal_ms": d4, "dense_tflops": c4.dense_flops / (d4 * 1e-3) / 1e12, "decode_us": k4 * 1e3,
+                        "frac_of_peak": c4.flops / (a4 * 1e-3) / 1e12 / peaks["bf16"], "marked_density": c4.flops / c4.dense_flops}
+        del c4
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic", "impl": "ours",
+        "config": {"workload": f"BASELINE.json configs[2] 32K context: {w.recipe}" if args.config == "32k" else w.name + ": " + w.recipe,
+                   "n_tokens": w.shape.n_tokens, "heads": f"{w.shape.n_q_heads}/{w.shape.n_kv_heads}", "head_dim": w.shape.head_dim,
+                   "l2": "inputs larger than L2 (Q+K+V+O = %d MB per step), no flush" % ((case.q.numel() * 2 + case.k.numel() * 2) * 2 // 2 ** 20),
+                   "parallelism": f"replicas x{world} (one prompt per rank, no collective)"},
+        "clocks": clocks, "gpu_launches": int(launches),
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": case.h2d_bytes, "d2h_bytes_per_step": case.d2h_bytes,
+                "ms_per_step": e2e_ms},
+        "roofline": {"bound": "tensor", "kernel": "sift_attention_kernel<128>", "achieved": achieved, "peak": peaks["bf16"],
+                     "unit": "TFLOP/s", "frac": achieved / peaks["bf16"], "traffic": None, "peak_source": peaks["src"] + " (burst)"},
+        "extra": extra,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        tf, dt, cores, what = cpu_oracle_sample(w)
+        out["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what, "seconds": dt}
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = wl.CONFIGS[args.config]()
+    vals, secs = [], []
+    what, cores = "", torch.get_num_threads()
+    for i in range(args.warmup + args.steps):
+        tf, dt, cores, what = cpu_oracle_sample(w, budget_rows=128, heads=(0,), seed=i)
+        if i >= args.warmup:
+            vals.append(tf)
+            secs.append(dt)
+    v = float(np.mean(vals))
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": float(np.mean(secs)) * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{w.name}: {w.recipe}", "n_tokens": w.shape.n_tokens},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": "each step: " + what},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="32k", choices=list(wl.CONFIGS))
+    ap.add_argument("--with-64k", dest="with_64k", action="store_true", default=True)
+    ap.add_argument("--no-64k", dest="with_64k", action="store_false")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
