@@ -6,8 +6,8 @@
 //   * persistent CTAs (one per SM) pull (q-head, M-block) work items, longest first, through an atomic counter;
 //   * an M-block is kNQ query tiles of 128 TMEM lanes of the same document and head: they share the head's cross
 //     list, so every gathered K/V tile in shared memory feeds kNQ accumulators;
-//   * warp roles: warp 0 = producer (TMA; `tile::gather4` for the row-granular cross keys, tiled boxes for local
-//     tiles and the dense query rows), warp 1 = tcgen05.mma issuer, warp 2 = TMEM allocator, warps 4.. = one softmax
+//   * warp roles: warp 0 = work-item fetch + Q tiles (TMA), warp 1 = tcgen05.mma issuer, warps 2/3 = K/V producers (tiled TMA
+//     boxes for local tiles and dense rows; TMA `tile::gather4` for the row-granular cross keys), warps 4.. = one softmax
 //     warpgroup per query tile (one row per thread, S read with tcgen05.ld, P written back to TMEM as bf16 and used
 //     as the A operand of the P*V MMA, lazy rescale of the TMEM-resident O accumulator);
 //   * S = Q K^T and O += P V are tcgen05.mma.kind::f16 (bf16 in, fp32 accumulate in TMEM).
@@ -18,6 +18,7 @@
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "sift_common.h"
@@ -32,6 +33,8 @@ constexpr int kBN = 128;                    // keys per step
 constexpr int kNumThreads = 128 + 128 * kNQ;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 with a stale max
 constexpr uint32_t kTmemCols = 512;
+constexpr int kRegsOther = 64;                                   // warps 0-3 after setmaxnreg.dec
+constexpr int kRegsSoftmax = (kNQ == 2) ? 216 : 232;              // softmax warps after setmaxnreg.inc
 
 struct AttnParams {
   // metadata (null in dense mode)
@@ -41,6 +44,10 @@ struct AttnParams {
   int32_t* counters;                                                         // [2]: next item, finished CTAs
   int32_t n_items, n_docs, n_tiles, cross_cap, local_cap, n_mblocks;
   int32_t dense;  // 1: every M-block is a DENSE item over n_tokens rows
+  int32_t gather_mode;      // 0: TMA tile::gather4 (default), 1: swizzled cp.async row gather (measured slower)
+  const char *k_ptr, *v_ptr;
+  int64_t k_row_bytes, v_row_bytes;
+  int32_t debug_no_gather;  // timing experiments only (wrong results): cross groups loaded as tiled boxes
   int32_t n_tokens, n_q_heads, n_kv_heads, tile;
   __nv_bfloat16* o;
   int64_t o_row_stride;
@@ -162,7 +169,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       mbar_init(bar(S::bPFull + q), 128);
       mbar_init(bar(S::bODone + q), 1);
     }
-    for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 1 + 128 * kNQ); }
+    for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 3 + 128 * kNQ); }
     fence_barrier_init();
     prefetch_tensormap(&tm_q); prefetch_tensormap(&tm_k); prefetch_tensormap(&tm_v);
     prefetch_tensormap(&tm_kg); prefetch_tensormap(&tm_vg);
@@ -176,10 +183,12 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   tc_fence_after();
   const uint32_t tmem_base = static_cast<uint32_t>(info[0]);
 
+  // register budget: the four non-softmax warps give registers to the softmax warpgroups (setmaxnreg at the top of
+  // every role branch so that it dominates the role's code)
   if (warp == 0) {
-    // ======================================= producer =======================================
-    uint32_t kst = 0, kph = 0, vst = 0, vph = 0;
-    const uint32_t q_smem = sbase + S::kQOff, k_smem = sbase + S::kKOff, v_smem = sbase + S::kVOff;
+    // ======================================= item fetch + Q producer =======================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
+    const uint32_t q_smem = sbase + S::kQOff;
     for (int it_n = 0;; ++it_n) {
       const int slot = it_n & 1;
       mbar_wait(bar(S::bItemEmpty + slot), ((it_n >> 1) & 1) ^ 1, 100);
@@ -210,44 +219,80 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                         it.row0[q]);
       }
       __syncwarp();
-      // ---- K/V tiles, one step at a time
+    }
+  } else if (warp == 2 || warp == 3) {
+    // ======================================= K (warp 2) / V (warp 3) producers =======================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
+    // Tiled steps: one TMA box per 64-column half.  Gathered (cross) steps: one `tile::gather4` per lane and half
+    // (4 rows x 128 B each, 32 lanes = 128 rows).  gather_mode 1 is the measured alternative: 16-byte cp.async per
+    // lane with the 128-byte swizzle applied by hand (chunk ^= row & 7); it is slower (profiles/gather_modes_r1.md).
+    const bool is_k = (warp == 2);
+    const int n_stages = is_k ? S::kKStages : S::kVStages;
+    const int b_full = is_k ? S::bKFull : S::bVFull, b_empty = is_k ? S::bKEmpty : S::bVEmpty;
+    const uint32_t ring = sbase + (is_k ? S::kKOff : S::kVOff);
+    const CUtensorMap* tm_tile = is_k ? &tm_k : &tm_v;
+    const CUtensorMap* tm_gath = is_k ? &tm_kg : &tm_vg;
+    const char* gbase = is_k ? p.k_ptr : p.v_ptr;
+    const int64_t row_bytes = is_k ? p.k_row_bytes : p.v_row_bytes;
+    uint32_t st = 0, ph = 0;
+    int pend = -1;   // stage whose cp.async group has been committed but not yet published
+    auto publish = [&](int stage) {
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(b_full + stage));
+    };
+    auto flush = [&]() {
+      if (pend >= 0) { cp_async_wait<0>(); publish(pend); pend = -1; }
+    };
+    for (int it_n = 0;; ++it_n) {
+      const int slot = it_n & 1;
+      mbar_wait(bar(S::bItemFull + slot), (it_n >> 1) & 1, 400);
+      const int code = info[1 + slot];
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(S::bItemEmpty + slot));
+      if (code < 0) break;
+      const Item it = load_item(p, code);
       auto emit = [&](bool gather, int src, int act, bool last) {
         // src: gather -> index of the first cross entry of the group; tiled -> first key row
         int4 r = make_int4(0, 0, 0, 0);
         if (gather) r = *reinterpret_cast<const int4*>(p.cross_idx + (int64_t)it.h * p.cross_cap + src + lane * 4);
-        mbar_wait(bar(S::bKEmpty + kst), kph ^ 1, 102);
-        if (lane == 0) {
-          info[4 + kst] = act | (last ? 4 : 0);
-          mbar_arrive_expect_tx(bar(S::bKFull + kst), S::kTileBytes);
+        if (pend >= 0 && !mbar_try_wait(bar(b_empty + st), ph ^ 1)) flush();
+        mbar_wait(bar(b_empty + st), ph ^ 1, 401);
+        if (is_k && lane == 0) info[4 + st] = act | (last ? 4 : 0);
+        const uint32_t dst = ring + st * S::kTileBytes;
+        if (gather && p.gather_mode == 1) {
+          const int sub = lane >> 3, c = lane & 7;
+          const char* col = gbase + (int64_t)it.kvh * (HD * 2) + c * 16;
+#pragma unroll 8
+          for (int j = 0; j < 32; ++j) {
+            const int v0 = __shfl_sync(0xffffffffu, r.x, j), v1 = __shfl_sync(0xffffffffu, r.y, j);
+            const int v2 = __shfl_sync(0xffffffffu, r.z, j), v3 = __shfl_sync(0xffffffffu, r.w, j);
+            const int v = sub == 0 ? v0 : (sub == 1 ? v1 : (sub == 2 ? v2 : v3));
+            const int row = 4 * j + sub;
+            const char* g = col + (int64_t)v * row_bytes;
+            const uint32_t d = dst + row * 128 + ((c ^ (row & 7)) << 4);
+#pragma unroll
+            for (int hf = 0; hf < S::kHalves; ++hf) cp_async16(d + hf * (kBN * 128), g + hf * 128);
+          }
+          cp_async_commit();
+          if (pend >= 0) { cp_async_wait<1>(); publish(pend); }
+          pend = st;
+        } else {
+          flush();
+          if (lane == 0) mbar_arrive_expect_tx(bar(b_full + st), S::kTileBytes);
+          __syncwarp();
+          if (gather) {
+#pragma unroll
+            for (int hf = 0; hf < S::kHalves; ++hf)
+              tma_gather4(dst + hf * (kBN * 128) + lane * 512, tm_gath, bar(b_full + st), it.kvh * HD + hf * 64, r.x, r.y,
+                          r.z, r.w);
+          } else if (lane == 0) {
+#pragma unroll
+            for (int hf = 0; hf < S::kHalves; ++hf)
+              tma_load_2d(dst + hf * (kBN * 128), tm_tile, bar(b_full + st), it.kvh * HD + hf * 64, src);
+          }
         }
-        __syncwarp();
-        const uint32_t kdst = k_smem + kst * S::kTileBytes;
-        if (gather) {
-#pragma unroll
-          for (int hf = 0; hf < S::kHalves; ++hf)
-            tma_gather4(kdst + hf * (kBN * 128) + lane * 512, &tm_kg, bar(S::bKFull + kst), it.kvh * HD + hf * 64, r.x,
-                        r.y, r.z, r.w);
-        } else if (lane == 0) {
-#pragma unroll
-          for (int hf = 0; hf < S::kHalves; ++hf)
-            tma_load_2d(kdst + hf * (kBN * 128), &tm_k, bar(S::bKFull + kst), it.kvh * HD + hf * 64, src);
-        }
-        if (++kst == S::kKStages) { kst = 0; kph ^= 1; }
-        mbar_wait(bar(S::bVEmpty + vst), vph ^ 1, 103);
-        if (lane == 0) mbar_arrive_expect_tx(bar(S::bVFull + vst), S::kTileBytes);
-        __syncwarp();
-        const uint32_t vdst = v_smem + vst * S::kTileBytes;
-        if (gather) {
-#pragma unroll
-          for (int hf = 0; hf < S::kHalves; ++hf)
-            tma_gather4(vdst + hf * (kBN * 128) + lane * 512, &tm_vg, bar(S::bVFull + vst), it.kvh * HD + hf * 64, r.x,
-                        r.y, r.z, r.w);
-        } else if (lane == 0) {
-#pragma unroll
-          for (int hf = 0; hf < S::kHalves; ++hf)
-            tma_load_2d(vdst + hf * (kBN * 128), &tm_v, bar(S::bVFull + vst), it.kvh * HD + hf * 64, src);
-        }
-        if (++vst == S::kVStages) { vst = 0; vph ^= 1; }
+        if (++st == (uint32_t)n_stages) { st = 0; ph ^= 1; }
       };
       if (it.is_dense) {
         int n[kNQ], total = 0;
@@ -264,7 +309,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
         for (int q = 0; q < kNQ; ++q) { present |= (it.rows[q] > 0) << q; nloc += it.lcnt[q]; }
         const int ngroups = (it.cp + kBN - 1) / kBN;
-        for (int g = 0; g < ngroups; ++g) emit(true, g * kBN, present, g == ngroups - 1 && nloc == 0);
+        for (int g = 0; g < ngroups; ++g) emit(!p.debug_no_gather, g * kBN, present, g == ngroups - 1 && nloc == 0);
         const int32_t* lidx = p.local_idx + (int64_t)it.h * p.local_cap;
         int pos[kNQ];
 #pragma unroll
@@ -286,9 +331,11 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           emit(false, p.tile_row0[t], act, remaining == 0);
         }
       }
+      flush();
     }
   } else if (warp == 1) {
     // ======================================= MMA issuer =======================================
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
     if (lane == 0) {
       uint32_t kst = 0, kph = 0, vst = 0, vph = 0, pph[kNQ];
 #pragma unroll
@@ -361,6 +408,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     }
   } else if (warp >= 4) {
     // ======================================= softmax warpgroups =======================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
     const int q = (warp - 4) >> 2;
     const int r = threadIdx.x - 128 - q * 128;             // row inside the query tile = TMEM lane
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
@@ -399,17 +447,31 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         sph ^= 1;
         tc_fence_after();
         float s[kBN];
+        {
+          uint32_t raw0[32], raw1[32], raw2[32], raw3[32];
+          tmem_ld32(s_addr + 0, raw0);
+          tmem_ld32(s_addr + 32, raw1);
+          tmem_ld32(s_addr + 64, raw2);
+          tmem_ld32(s_addr + 96, raw3);
+          tmem_wait_ld();
 #pragma unroll
-        for (int c = 0; c < kBN / 32; ++c) tmem_ld32(s_addr + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
-        tmem_wait_ld();
+          for (int c = 0; c < 32; ++c) {
+            s[c] = __uint_as_float(raw0[c]); s[32 + c] = __uint_as_float(raw1[c]);
+            s[64 + c] = __uint_as_float(raw2[c]); s[96 + c] = __uint_as_float(raw3[c]);
+          }
+        }
         if (causal || n_valid < kBN) {
           const int lim = causal ? min(n_valid, r - kdelta + 1) : n_valid;   // columns [0, lim) are allowed
 #pragma unroll
           for (int c = 0; c < kBN; ++c) s[c] = (c < lim) ? s[c] : -INFINITY;
         }
-        float mx = s[0];
+        float mx4[4] = {s[0], s[1], s[2], s[3]};                  // four independent chains
 #pragma unroll
-        for (int c = 1; c < kBN; ++c) mx = fmaxf(mx, s[c]);
+        for (int c = 4; c < kBN; c += 4) {
+          mx4[0] = fmaxf(mx4[0], s[c]); mx4[1] = fmaxf(mx4[1], s[c + 1]);
+          mx4[2] = fmaxf(mx4[2], s[c + 2]); mx4[3] = fmaxf(mx4[3], s[c + 3]);
+        }
+        const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
         const float m_new = fmaxf(m, mx);
         const bool need = (m_new - m) * sl > kRescaleThreshold;   // (-inf) - (-inf) = NaN -> false
         if (__any_sync(0xffffffffu, need)) {
@@ -432,7 +494,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           }
         }
         const float neg_m = (m == -INFINITY) ? 0.f : -m * sl;
-        float sum = 0.f;
+        float sum0 = 0.f, sum1 = 0.f;
 #pragma unroll
         for (int c = 0; c < kBN / 32; ++c) {
           uint32_t pk[16];
@@ -440,7 +502,8 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           for (int i = 0; i < 16; ++i) {
             const float p0 = ex2(fmaf(s[c * 32 + 2 * i], sl, neg_m));
             const float p1 = ex2(fmaf(s[c * 32 + 2 * i + 1], sl, neg_m));
-            sum += p0 + p1;
+            sum0 += p0;
+            sum1 += p1;
             pk[i] = pack_bf16x2(p0, p1);
           }
           // P (bf16) overwrites the first 64 columns of S: 16 packed columns per 32 keys
@@ -450,7 +513,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                 "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
                 "r"(pk[15]) : "memory");
         }
-        l += sum;
+        l += sum0 + sum1;
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(bar(S::bPFull + q));
@@ -546,6 +609,9 @@ static int launch_attention(AttnParams& p, const void* Q, const void* K, const v
                             cudaStream_t st) {
   CUtensorMap tq, tk, tv, tkg, tvg;
   int rc;
+  p.k_ptr = static_cast<const char*>(K); p.v_ptr = static_cast<const char*>(V);
+  p.k_row_bytes = ks * 2; p.v_row_bytes = vs * 2;
+  { const char* e = getenv("SIFT_GATHER_MODE"); p.gather_mode = (e && e[0] == '1') ? 1 : 0; }  // 1 = cp.async experiment
   const int64_t n = p.n_tokens;
   if ((rc = make_map(&tq, Q, n, (int64_t)p.n_q_heads * HD, qs, kBM))) return rc;
   if ((rc = make_map(&tk, K, n, (int64_t)p.n_kv_heads * HD, ks, kBN))) return rc;
@@ -610,6 +676,7 @@ extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, co
   p.n_items = lay.n_items; p.n_docs = D; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap;
   p.local_cap = lay.local_cap; p.n_mblocks = lay.n_mblocks;
   p.dense = 0;
+  { const char* e = getenv("SIFT_DEBUG_NO_GATHER"); p.debug_no_gather = (e && e[0] == '1'); }
   p.n_tokens = shape->doc_offsets[D] + shape->query_len;
   p.n_q_heads = Hq; p.n_kv_heads = shape->n_kv_heads; p.tile = shape->tile;
   p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
