@@ -30,11 +30,25 @@ using namespace ptx;
 constexpr int kNQ = SIFT_Q_TILES_PER_ITEM;  // query tiles per work item
 constexpr int kBM = 128;                    // rows of one query tile = TMEM lanes
 constexpr int kBN = 128;                    // keys per step
-constexpr int kNumThreads = 128 + 128 * kNQ;
+constexpr int kNumThreads = 256 + 128 * kNQ;        // warps 0-3 control/K, softmax warpgroups, 2 V-producer warps, 2 idle
+                                                   // (4 warps per SM sub-partition: registers are pooled per sub-partition)
+constexpr int kFirstVWarp = 4 + 4 * kNQ;
+constexpr int kProducerThreads = 64;              // per operand
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 with a stale max
 constexpr uint32_t kTmemCols = 512;
-constexpr int kRegsOther = 64;                                   // warps 0-3 after setmaxnreg.dec
-constexpr int kRegsSoftmax = (kNQ == 2) ? 216 : 232;              // softmax warps after setmaxnreg.inc
+
+constexpr int kRegsEntry = (kNQ == 2) ? 128 : 168;               // what __launch_bounds__(kNumThreads, 1) yields
+constexpr int kRegsOther = 48;                                   // non-softmax warps after setmaxnreg.dec
+constexpr int kRegsSoftmax = (kNQ == 2) ? 208 : 232;              // softmax warps after setmaxnreg.inc
+
+static_assert(kNQ * kRegsSoftmax + 2 * kRegsOther <= (kNumThreads / 128) * kRegsEntry,
+              "setmaxnreg budget exceeds the register pool the CTA is launched with (softmax warps would block)");
+
+#ifdef SIFT_NO_CFENCE
+#define CFENCE() do {} while (0)
+#else
+#define CFENCE() fence_proxy_async()
+#endif
 
 struct AttnParams {
   // metadata (null in dense mode)
@@ -43,8 +57,9 @@ struct AttnParams {
   const int32_t* sched;                                                      // already offset to the layer
   int32_t* counters;                                                         // [2]: next item, finished CTAs
   int32_t n_items, n_docs, n_tiles, cross_cap, local_cap, n_mblocks;
+  int32_t zero;   // always 0 (see the TMEM address note in the kernel)
   int32_t dense;  // 1: every M-block is a DENSE item over n_tokens rows
-  int32_t gather_mode;      // 0: TMA tile::gather4 (default), 1: swizzled cp.async row gather (measured slower)
+  int32_t gather_mode;      // 0: swizzled cp.async row gather (default), 1: TMA tile::gather4
   const char *k_ptr, *v_ptr;
   int64_t k_row_bytes, v_row_bytes;
   int32_t debug_no_gather;  // timing experiments only (wrong results): cross groups loaded as tiled boxes
@@ -155,21 +170,21 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   const uint32_t bar0 = sbase + S::kBarOff;
   auto bar = [&](int i) -> uint32_t { return bar0 + i * 8; };
   volatile int32_t* info = reinterpret_cast<volatile int32_t*>(sgen + S::kInfoOff);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;   // warp-uniform role id
   constexpr uint32_t idesc_qk = umma_idesc_bf16(kBM, kBN, 0, 0);
   constexpr uint32_t idesc_pv = umma_idesc_bf16(kBM, HD, 0, 1);
 
   if (warp == 0 && lane == 0) {
     mbar_init(bar(S::bQFull), 1);
     mbar_init(bar(S::bQEmpty), 1);
-    for (int i = 0; i < S::kKStages; ++i) { mbar_init(bar(S::bKFull + i), 1); mbar_init(bar(S::bKEmpty + i), 1); }
-    for (int i = 0; i < S::kVStages; ++i) { mbar_init(bar(S::bVFull + i), 1); mbar_init(bar(S::bVEmpty + i), 1); }
+    for (int i = 0; i < S::kKStages; ++i) { mbar_init(bar(S::bKFull + i), kProducerThreads); mbar_init(bar(S::bKEmpty + i), 1); }
+    for (int i = 0; i < S::kVStages; ++i) { mbar_init(bar(S::bVFull + i), kProducerThreads); mbar_init(bar(S::bVEmpty + i), 1); }
     for (int q = 0; q < kNQ; ++q) {
       mbar_init(bar(S::bSFull + q), 1);
       mbar_init(bar(S::bPFull + q), 128);
       mbar_init(bar(S::bODone + q), 1);
     }
-    for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 3 + 128 * kNQ); }
+    for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 5 + 128 * kNQ); }
     fence_barrier_init();
     prefetch_tensormap(&tm_q); prefetch_tensormap(&tm_k); prefetch_tensormap(&tm_v);
     prefetch_tensormap(&tm_kg); prefetch_tensormap(&tm_vg);
@@ -181,7 +196,13 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_base = static_cast<uint32_t>(info[0]);
+  // The CTA owns the whole TMEM (512 columns, 1 CTA per SM), so the allocation starts at column 0, lane 0: addresses
+  // below are compile-time constants (uniform registers for the MMA issuer).
+  if (info[0] != 0) { if (threadIdx.x == 0) printf("sift: unexpected TMEM base %d\n", (int)info[0]); __trap(); }
+  // (p.zero is a kernel parameter that is always 0: an operand ptxas must treat as a uniform run-time value, which
+  // keeps the tcgen05 address operands in uniform registers instead of a vector-register constant + R2UR.)
+  constexpr uint32_t tmem_base = 0;
+  const uint32_t kTmemS = (uint32_t)p.zero, kTmemO = (uint32_t)p.zero + 256;
 
   // register budget: the four non-softmax warps give registers to the softmax warpgroups (setmaxnreg at the top of
   // every role branch so that it dominates the role's code)
@@ -220,30 +241,30 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       }
       __syncwarp();
     }
-  } else if (warp == 2 || warp == 3) {
-    // ======================================= K (warp 2) / V (warp 3) producers =======================================
+  } else if (warp == 2 || warp == 3 || warp == kFirstVWarp || warp == kFirstVWarp + 1) {
+    // ======================================= K (warps 2,3) / V (last two warps) producers =======================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
-    // Tiled steps: one TMA box per 64-column half.  Gathered (cross) steps: one `tile::gather4` per lane and half
-    // (4 rows x 128 B each, 32 lanes = 128 rows).  gather_mode 1 is the measured alternative: 16-byte cp.async per
-    // lane with the 128-byte swizzle applied by hand (chunk ^= row & 7); it is slower (profiles/gather_modes_r1.md).
-    const bool is_k = (warp == 2);
+    // 64 threads per operand.  Tiled steps (local tiles, dense rows): one thread issues one TMA box per 64-column half.
+    // Gathered steps (cross keys, row-granular): gather_mode 0 (default) = every thread copies 16-byte pieces of the
+    // listed rows with cp.async, applying the 128-byte swizzle by hand (chunk ^= row & 7) so that the landed image is
+    // what a tiled box would have written; completion is signalled by cp.async.mbarrier.arrive.  gather_mode 1 = TMA
+    // `tile::gather4`, one per lane and half; it is issue-bound at ~70 clk per instruction and warp
+    // (profiles/r1_gather_modes.md) and kept for comparison.
+    const bool is_k = warp < 4;
+    const int ptid = is_k ? (int)threadIdx.x - 64 : (int)threadIdx.x - kFirstVWarp * 32;
     const int n_stages = is_k ? S::kKStages : S::kVStages;
     const int b_full = is_k ? S::bKFull : S::bVFull, b_empty = is_k ? S::bKEmpty : S::bVEmpty;
     const uint32_t ring = sbase + (is_k ? S::kKOff : S::kVOff);
     const CUtensorMap* tm_tile = is_k ? &tm_k : &tm_v;
     const CUtensorMap* tm_gath = is_k ? &tm_kg : &tm_vg;
-    const char* gbase = is_k ? p.k_ptr : p.v_ptr;
     const int64_t row_bytes = is_k ? p.k_row_bytes : p.v_row_bytes;
+    constexpr int CH = HD / 8;          // 16-byte chunks per row
+    constexpr int RPP = 64 / CH;        // rows per pass of the 64 threads
+    constexpr int PASSES = kBN / RPP;
+    constexpr int PCH = 16;             // passes per batch of index loads
+    const int c = ptid % CH, rr = ptid / CH;
+    const uint32_t dst_thr = (uint32_t)((c >> 3) * (kBN * 128) + rr * 128);
     uint32_t st = 0, ph = 0;
-    int pend = -1;   // stage whose cp.async group has been committed but not yet published
-    auto publish = [&](int stage) {
-      fence_proxy_async();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(b_full + stage));
-    };
-    auto flush = [&]() {
-      if (pend >= 0) { cp_async_wait<0>(); publish(pend); pend = -1; }
-    };
     for (int it_n = 0;; ++it_n) {
       const int slot = it_n & 1;
       mbar_wait(bar(S::bItemFull + slot), (it_n >> 1) & 1, 400);
@@ -252,44 +273,48 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       if (lane == 0) mbar_arrive(bar(S::bItemEmpty + slot));
       if (code < 0) break;
       const Item it = load_item(p, code);
+      const char* col = (is_k ? p.k_ptr : p.v_ptr) + (int64_t)it.kvh * (HD * 2) + c * 16;
       auto emit = [&](bool gather, int src, int act, bool last) {
         // src: gather -> index of the first cross entry of the group; tiled -> first key row
-        int4 r = make_int4(0, 0, 0, 0);
-        if (gather) r = *reinterpret_cast<const int4*>(p.cross_idx + (int64_t)it.h * p.cross_cap + src + lane * 4);
-        if (pend >= 0 && !mbar_try_wait(bar(b_empty + st), ph ^ 1)) flush();
-        mbar_wait(bar(b_empty + st), ph ^ 1, 401);
-        if (is_k && lane == 0) info[4 + st] = act | (last ? 4 : 0);
-        const uint32_t dst = ring + st * S::kTileBytes;
-        if (gather && p.gather_mode == 1) {
-          const int sub = lane >> 3, c = lane & 7;
-          const char* col = gbase + (int64_t)it.kvh * (HD * 2) + c * 16;
-#pragma unroll 8
-          for (int j = 0; j < 32; ++j) {
-            const int v0 = __shfl_sync(0xffffffffu, r.x, j), v1 = __shfl_sync(0xffffffffu, r.y, j);
-            const int v2 = __shfl_sync(0xffffffffu, r.z, j), v3 = __shfl_sync(0xffffffffu, r.w, j);
-            const int v = sub == 0 ? v0 : (sub == 1 ? v1 : (sub == 2 ? v2 : v3));
-            const int row = 4 * j + sub;
-            const char* g = col + (int64_t)v * row_bytes;
-            const uint32_t d = dst + row * 128 + ((c ^ (row & 7)) << 4);
+        const uint32_t full = bar(b_full + st), dst = ring + st * S::kTileBytes;
+        if (gather && p.gather_mode == 0) {
+          const int32_t* ip = p.cross_idx + (int64_t)it.h * p.cross_cap + src + rr;
+          int rows[PCH];
 #pragma unroll
-            for (int hf = 0; hf < S::kHalves; ++hf) cp_async16(d + hf * (kBN * 128), g + hf * 128);
+          for (int j = 0; j < PCH; ++j) rows[j] = __ldg(ip + j * RPP);
+          mbar_wait(bar(b_empty + st), ph ^ 1, 401);
+          if (is_k && ptid == 0) info[4 + st] = act | (last ? 4 : 0);
+#pragma unroll
+          for (int p0 = 0; p0 < PASSES; p0 += PCH) {
+#pragma unroll
+            for (int j = 0; j < PCH; ++j) {
+              const int row = (p0 + j) * RPP + rr;
+              cp_async16(dst + dst_thr + (p0 + j) * RPP * 128 + (((c & 7) ^ (row & 7)) << 4), col + (int64_t)rows[j] * row_bytes);
+            }
+            if (p0 + PCH < PASSES) {
+#pragma unroll
+              for (int j = 0; j < PCH; ++j) rows[j] = __ldg(ip + (p0 + PCH + j) * RPP);
+            }
           }
-          cp_async_commit();
-          if (pend >= 0) { cp_async_wait<1>(); publish(pend); }
-          pend = st;
+          cp_async_mbar_arrive_noinc(full);
         } else {
-          flush();
-          if (lane == 0) mbar_arrive_expect_tx(bar(b_full + st), S::kTileBytes);
-          __syncwarp();
+          int4 r = make_int4(0, 0, 0, 0);
+          if (gather) r = *reinterpret_cast<const int4*>(p.cross_idx + (int64_t)it.h * p.cross_cap + src + lane * 4);
+          mbar_wait(bar(b_empty + st), ph ^ 1, 401);
+          if (ptid == 0) {
+            if (is_k) info[4 + st] = act | (last ? 4 : 0);
+            mbar_arrive_expect_tx(full, S::kTileBytes);
+          } else {
+            mbar_arrive(full);
+          }
           if (gather) {
+            const int hf = ptid >> 5;      // the first warp gathers columns 0..63, the second 64..127
+            if (hf < S::kHalves)
+              tma_gather4(dst + hf * (kBN * 128) + lane * 512, tm_gath, full, it.kvh * HD + hf * 64, r.x, r.y, r.z, r.w);
+          } else if (ptid == 0) {
 #pragma unroll
             for (int hf = 0; hf < S::kHalves; ++hf)
-              tma_gather4(dst + hf * (kBN * 128) + lane * 512, tm_gath, bar(b_full + st), it.kvh * HD + hf * 64, r.x, r.y,
-                          r.z, r.w);
-          } else if (lane == 0) {
-#pragma unroll
-            for (int hf = 0; hf < S::kHalves; ++hf)
-              tma_load_2d(dst + hf * (kBN * 128), tm_tile, bar(b_full + st), it.kvh * HD + hf * 64, src);
+              tma_load_2d(dst + hf * (kBN * 128), tm_tile, full, it.kvh * HD + hf * 64, src);
           }
         }
         if (++st == (uint32_t)n_stages) { st = 0; ph ^= 1; }
@@ -331,82 +356,107 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           emit(false, p.tile_row0[t], act, remaining == 0);
         }
       }
-      flush();
     }
   } else if (warp == 1) {
     // ======================================= MMA issuer =======================================
+    // The whole warp walks the loop so that every address / descriptor is warp-uniform (values read from shared
+    // memory are re-broadcast with shfl so that ptxas keeps them in uniform registers); one elected lane issues.
+    // With a divergent `if (lane == 0)` around the loop every tcgen05.mma operand took an R2UR round trip and the
+    // issuing thread itself became the bottleneck (profiles/r1_mma_issue.md).
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
-    if (lane == 0) {
-      uint32_t kst = 0, kph = 0, vst = 0, vph = 0, pph[kNQ];
+    uint32_t kst = 0, kph = 0, vst = 0, vph = 0, pph[kNQ];
 #pragma unroll
-      for (int q = 0; q < kNQ; ++q) pph[q] = 0;
-      const uint32_t q_smem = sbase + S::kQOff, k_smem = sbase + S::kKOff, v_smem = sbase + S::kVOff;
-      for (int it_n = 0;; ++it_n) {
-        const int slot = it_n & 1;
-        mbar_wait(bar(S::bItemFull + slot), (it_n >> 1) & 1, 200);
-        const int code = info[1 + slot];
-        mbar_arrive(bar(S::bItemEmpty + slot));
-        if (code < 0) break;
+    for (int q = 0; q < kNQ; ++q) pph[q] = 0;
+    const uint32_t q_smem = sbase + S::kQOff, k_smem = sbase + S::kKOff, v_smem = sbase + S::kVOff;
+    for (int it_n = 0;; ++it_n) {
+      const int slot = it_n & 1;
+      mbar_wait(bar(S::bItemFull + slot), (it_n >> 1) & 1, 200);
+      const int code = __shfl_sync(0xffffffffu, (int)info[1 + slot], 0);
+      if (lane == 0) mbar_arrive(bar(S::bItemEmpty + slot));
+      if (code < 0) break;
+      int has_steps;
+      {
         const Item it = load_item(p, code);
-        bool has_steps = it.is_dense || it.cp > 0;
+        bool hs = it.is_dense || it.cp > 0;
 #pragma unroll
-        for (int q = 0; q < kNQ; ++q) has_steps = has_steps || it.lcnt[q] > 0;
-        mbar_wait(bar(S::bQFull), it_n & 1, 201);
-        if (!has_steps) { mbar_arrive(bar(S::bQEmpty)); continue; }
+        for (int q = 0; q < kNQ; ++q) hs = hs || it.lcnt[q] > 0;
+        has_steps = __shfl_sync(0xffffffffu, (int)hs, 0);
+      }
+      mbar_wait(bar(S::bQFull), it_n & 1, 201);
+      if (!has_steps) {
+        if (lane == 0) mbar_arrive(bar(S::bQEmpty));
+        continue;
+      }
+      tc_fence_after();
+      // PV of step j-1 is issued in iteration j, right before Q K^T of step j for the same query tile (tensor-pipe
+      // order PV0 QK0 PV1 QK1: the softmax of one tile overlaps the MMAs of the other).  `pending`, `act` and
+      // `fresh` come from shared memory, which ptxas cannot prove warp-uniform: they only steer branches, while every
+      // MMA operand is built from uniform counters (kst, vst, j) and constants.
+#define SIFT_ISSUE_PV(q, ACC)                                                                                    \
+  if (elect_one()) {                                                                                             \
+    _Pragma("unroll") for (int k = 0; k < kBN / 16; ++k)                                                         \
+        umma_ts(kTmemO + q * 128, kTmemS + q * 128 + k * 8, v_desc<HD>(vt, k), idesc_pv, (ACC) | (k > 0));      \
+    umma_commit(bar(S::bODone + q));                                                                             \
+  }                                                                                                              \
+  __syncwarp();
+#define SIFT_PV_STEP(q)                                                                                          \
+  if (pending & (1 << q)) {                                                                                      \
+    mbar_wait(bar(S::bPFull + q), pph[q], 202);                                                                  \
+    pph[q] ^= 1;                                                                                                 \
+    tc_fence_after();                                                                                            \
+    if (fresh & (1 << q)) { SIFT_ISSUE_PV(q, 0) } else { SIFT_ISSUE_PV(q, 1) }                                   \
+    fresh &= ~(1 << q);                                                                                          \
+  }
+      int pending = 0, fresh = (1 << kNQ) - 1;   // fresh bit q: the next P V of tile q overwrites O instead of accumulating
+      bool last = false;
+      for (int j = 0; !last; ++j) {
+        mbar_wait(bar(S::bKFull + kst), kph, 204);
+        const int inf = info[4 + kst];
+        const int act = inf & 3;
+        last = (inf & 4) != 0;
+        const uint32_t kt = k_smem + kst * S::kTileBytes, vt = v_smem + vst * S::kTileBytes;
+        if (j > 0) mbar_wait(bar(S::bVFull + vst), vph, 203);
+        CFENCE();   // cp.async-gathered tiles were written through the generic proxy
         tc_fence_after();
-        int pending = 0;
-        uint32_t accum[kNQ];
 #pragma unroll
-        for (int q = 0; q < kNQ; ++q) accum[q] = 0;
-        auto flush_pv = [&](int q, bool& v_waited) {
-          mbar_wait(bar(S::bPFull + q), pph[q], 202);
-          pph[q] ^= 1;
-          if (!v_waited) { mbar_wait(bar(S::bVFull + vst), vph, 203); v_waited = true; }
-          tc_fence_after();
-          const uint32_t vt = v_smem + vst * S::kTileBytes;
-#pragma unroll
-          for (int k = 0; k < kBN / 16; ++k)
-            umma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + k * 8, v_desc<HD>(vt, k), idesc_pv, accum[q] | (k > 0));
-          accum[q] = 1;
-          umma_commit(bar(S::bODone + q));
-        };
-        bool last = false;
-        while (!last) {
-          mbar_wait(bar(S::bKFull + kst), kph, 204);
-          const int inf = info[4 + kst];
-          const int act = inf & 3;
-          last = (inf & 4) != 0;
-          tc_fence_after();
-          bool v_waited = false;
-          const uint32_t kt = k_smem + kst * S::kTileBytes;
-#pragma unroll
-          for (int q = 0; q < kNQ; ++q) {
-            if (pending & (1 << q)) flush_pv(q, v_waited);
-            if (act & (1 << q)) {
+        for (int q = 0; q < kNQ; ++q) {
+          SIFT_PV_STEP(q)
+          if (act & (1 << q)) {
+            if (elect_one()) {
 #pragma unroll
               for (int k = 0; k < HD / 16; ++k)
-                umma_ss(tmem_base + q * 128, kmajor_desc<HD>(q_smem + q * S::kTileBytes, k), kmajor_desc<HD>(kt, k), idesc_qk, k > 0);
+                umma_ss(kTmemS + q * 128, kmajor_desc<HD>(q_smem + q * S::kTileBytes, k), kmajor_desc<HD>(kt, k), idesc_qk, k > 0);
               umma_commit(bar(S::bSFull + q));
             }
+            __syncwarp();
           }
-          if (pending) {
-            umma_commit(bar(S::bVEmpty + vst));
-            if (++vst == S::kVStages) { vst = 0; vph ^= 1; }
-          }
-          umma_commit(bar(S::bKEmpty + kst));
-          if (++kst == S::kKStages) { kst = 0; kph ^= 1; }
-          pending = act;
         }
-        umma_commit(bar(S::bQEmpty));   // every Q K^T of this item has been issued
-        bool v_waited = false;
+        if (elect_one()) {
+          if (j > 0) umma_commit(bar(S::bVEmpty + vst));
+          umma_commit(bar(S::bKEmpty + kst));
+        }
+        __syncwarp();
+        if (j > 0) { if (++vst == S::kVStages) { vst = 0; vph ^= 1; } }
+        if (++kst == S::kKStages) { kst = 0; kph ^= 1; }
+        pending = act;
+      }
+      if (elect_one()) umma_commit(bar(S::bQEmpty));   // every Q K^T of this item has been issued
+      __syncwarp();
+      {
+        const uint32_t vt = v_smem + vst * S::kTileBytes;
+        mbar_wait(bar(S::bVFull + vst), vph, 203);
+        CFENCE();
+        tc_fence_after();
 #pragma unroll
-        for (int q = 0; q < kNQ; ++q)
-          if (pending & (1 << q)) flush_pv(q, v_waited);
-        umma_commit(bar(S::bVEmpty + vst));
+        for (int q = 0; q < kNQ; ++q) { SIFT_PV_STEP(q) }
+        if (elect_one()) umma_commit(bar(S::bVEmpty + vst));
+        __syncwarp();
         if (++vst == S::kVStages) { vst = 0; vph ^= 1; }
       }
+#undef SIFT_PV_STEP
+#undef SIFT_ISSUE_PV
     }
-  } else if (warp >= 4) {
+  } else if (warp >= 4 && warp < kFirstVWarp) {
     // ======================================= softmax warpgroups =======================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
     const int q = (warp - 4) >> 2;
@@ -446,6 +496,9 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         mbar_wait(bar(S::bSFull + q), sph, 301);
         sph ^= 1;
         tc_fence_after();
+#if defined(SIFT_ABL) && SIFT_ABL == 2
+        tc_fence_before(); mbar_arrive(bar(S::bPFull + q)); ++pv_cnt; l = 1.f; m = 0.f; continue;
+#endif
         float s[kBN];
         {
           uint32_t raw0[32], raw1[32], raw2[32], raw3[32];
@@ -500,8 +553,13 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           uint32_t pk[16];
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
+#if defined(SIFT_ABL) && SIFT_ABL == 1
+            const float p0 = fmaf(s[c * 32 + 2 * i], sl, neg_m);
+            const float p1 = fmaf(s[c * 32 + 2 * i + 1], sl, neg_m);
+#else
             const float p0 = ex2(fmaf(s[c * 32 + 2 * i], sl, neg_m));
             const float p1 = ex2(fmaf(s[c * 32 + 2 * i + 1], sl, neg_m));
+#endif
             sum0 += p0;
             sum1 += p1;
             pk[i] = pack_bf16x2(p0, p1);
@@ -552,6 +610,8 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       if (row_ok && p.lse != nullptr)
         p.lse[(int64_t)it.h * p.n_tokens + grow] = (l > 0.f) ? (m * sl + log2f(l)) * 0.6931471805599453f : -INFINITY;
     }
+  } else {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));   // idle warps only donate registers
   }
 
   tc_fence_before();
@@ -611,7 +671,7 @@ static int launch_attention(AttnParams& p, const void* Q, const void* K, const v
   int rc;
   p.k_ptr = static_cast<const char*>(K); p.v_ptr = static_cast<const char*>(V);
   p.k_row_bytes = ks * 2; p.v_row_bytes = vs * 2;
-  { const char* e = getenv("SIFT_GATHER_MODE"); p.gather_mode = (e && e[0] == '1') ? 1 : 0; }  // 1 = cp.async experiment
+  { const char* e = getenv("SIFT_GATHER_MODE"); p.gather_mode = (e && e[0] == '1') ? 1 : 0; }  // 1 = TMA gather4 (comparison)
   const int64_t n = p.n_tokens;
   if ((rc = make_map(&tq, Q, n, (int64_t)p.n_q_heads * HD, qs, kBM))) return rc;
   if ((rc = make_map(&tk, K, n, (int64_t)p.n_kv_heads * HD, ks, kBN))) return rc;
