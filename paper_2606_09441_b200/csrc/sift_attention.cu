@@ -20,6 +20,7 @@
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
+#include <type_traits>
 
 #include "sift_common.h"
 #include "sm100_ptx.cuh"
@@ -28,6 +29,7 @@ namespace sift {
 using namespace ptx;
 
 constexpr int kNQ = SIFT_Q_TILES_PER_ITEM;  // query tiles per work item
+static_assert(kNQ == 2, "the softmax warpgroups split the columns of one tile and alternate between two tiles");
 constexpr int kBM = 128;                    // rows of one query tile = TMEM lanes
 constexpr int kBN = 128;                    // keys per step
 constexpr int kNumThreads = 256 + 128 * kNQ;        // warps 0-3 control/K, softmax warpgroups, 2 V-producer warps, 2 idle
@@ -59,7 +61,7 @@ struct AttnParams {
   int32_t n_items, n_docs, n_tiles, cross_cap, local_cap, n_mblocks;
   int32_t zero;   // always 0 (see the TMEM address note in the kernel)
   int32_t dense;  // 1: every M-block is a DENSE item over n_tokens rows
-  int32_t gather_mode;      // 0: swizzled cp.async row gather (default), 1: TMA tile::gather4
+  int32_t gather_mode;      // 0: TMA tile::gather4 (default), 1: swizzled cp.async row gather
   const char *k_ptr, *v_ptr;
   int64_t k_row_bytes, v_row_bytes;
   int32_t debug_no_gather;  // timing experiments only (wrong results): cross groups loaded as tiled boxes
@@ -89,7 +91,9 @@ struct Smem {
   static constexpr int kNumBars = bItemEmpty + 2;
   static constexpr int kInfoOff = kBarOff + ((kNumBars * 8 + 15) / 16) * 16;
   // info words: [0] tmem base, [1..2] item ring, [4 .. 4+kKStages) per-K-stage step info
-  static constexpr int kBytes = kInfoOff + 64 + 1024;      // + slack for the manual 1024-byte alignment
+  static constexpr int kXchgOff = kInfoOff + 64;           // row max / row sum exchange between the two column halves
+  static constexpr int kBytes = kXchgOff + 2 * 2 * 128 * 4;
+  static_assert(kBytes <= 227 * 1024, "shared memory budget");
 };
 
 // One work item as every role sees it.
@@ -157,16 +161,32 @@ __device__ __forceinline__ uint64_t v_desc(uint32_t tile_addr, int k) {
   return umma_desc_sw128(tile_addr + k * 2048, kBN * 128, 1024);
 }
 
+// compile-time unrolled issue loops (the TMEM offsets must be immediates)
+template <int HD, int Q, int ACC, int K = 0>
+__device__ __forceinline__ void issue_pv(uint32_t tz, uint32_t vt, uint32_t idesc) {
+  if constexpr (K < kBN / 16) {
+    umma_ts_off<256 + Q * 128, Q * 128 + K * 8>(tz, v_desc<HD>(vt, K), idesc, (ACC) | (K > 0));
+    issue_pv<HD, Q, ACC, K + 1>(tz, vt, idesc);
+  }
+}
+template <int HD, int Q, int K = 0>
+__device__ __forceinline__ void issue_qk(uint32_t tz, uint32_t qt, uint32_t kt, uint32_t idesc) {
+  if constexpr (K < HD / 16) {
+    umma_ss_off<Q * 128>(tz, kmajor_desc<HD>(qt, K), kmajor_desc<HD>(kt, K), idesc, K > 0);
+    issue_qk<HD, Q, K + 1>(tz, qt, kt, idesc);
+  }
+}
+
 template <int HD>
 __global__ void __launch_bounds__(kNumThreads, 1)
 sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                       const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_kg,
                       const __grid_constant__ CUtensorMap tm_vg, const AttnParams p) {
   using S = Smem<HD>;
-  extern __shared__ uint8_t smem_raw[];
-  const uint32_t raw = smem_u32(smem_raw);
-  const uint32_t sbase = (raw + 1023u) & ~1023u;
-  uint8_t* sgen = smem_raw + (sbase - raw);
+  extern __shared__ __align__(1024) uint8_t smem_raw[];    // the only shared memory of the kernel: starts 1024-aligned
+  const uint32_t sbase = smem_u32(smem_raw);
+  uint8_t* sgen = smem_raw;
+  if ((sbase & 1023u) != 0) { if (threadIdx.x == 0) printf("sift: dynamic shared memory not 1024-byte aligned\n"); __trap(); }
   const uint32_t bar0 = sbase + S::kBarOff;
   auto bar = [&](int i) -> uint32_t { return bar0 + i * 8; };
   volatile int32_t* info = reinterpret_cast<volatile int32_t*>(sgen + S::kInfoOff);
@@ -181,7 +201,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     for (int i = 0; i < S::kVStages; ++i) { mbar_init(bar(S::bVFull + i), kProducerThreads); mbar_init(bar(S::bVEmpty + i), 1); }
     for (int q = 0; q < kNQ; ++q) {
       mbar_init(bar(S::bSFull + q), 1);
-      mbar_init(bar(S::bPFull + q), 128);
+      mbar_init(bar(S::bPFull + q), 256);   // both column halves
       mbar_init(bar(S::bODone + q), 1);
     }
     for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 5 + 128 * kNQ); }
@@ -202,7 +222,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   // (p.zero is a kernel parameter that is always 0: an operand ptxas must treat as a uniform run-time value, which
   // keeps the tcgen05 address operands in uniform registers instead of a vector-register constant + R2UR.)
   constexpr uint32_t tmem_base = 0;
-  const uint32_t kTmemS = (uint32_t)p.zero, kTmemO = (uint32_t)p.zero + 256;
+  const uint32_t tz = (uint32_t)p.zero;
 
   // register budget: the four non-softmax warps give registers to the softmax warpgroups (setmaxnreg at the top of
   // every role branch so that it dominates the role's code)
@@ -245,11 +265,12 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     // ======================================= K (warps 2,3) / V (last two warps) producers =======================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
     // 64 threads per operand.  Tiled steps (local tiles, dense rows): one thread issues one TMA box per 64-column half.
-    // Gathered steps (cross keys, row-granular): gather_mode 0 (default) = every thread copies 16-byte pieces of the
-    // listed rows with cp.async, applying the 128-byte swizzle by hand (chunk ^= row & 7) so that the landed image is
-    // what a tiled box would have written; completion is signalled by cp.async.mbarrier.arrive.  gather_mode 1 = TMA
-    // `tile::gather4`, one per lane and half; it is issue-bound at ~70 clk per instruction and warp
-    // (profiles/r1_gather_modes.md) and kept for comparison.
+    // Gathered steps (cross keys, row-granular): gather_mode 0 (default) = TMA `tile::gather4`, one instruction per
+    // lane and 64-column half (ptxas serialises the 32 lanes of a gather4 into a loop of uniform-datapath issues,
+    // ~70 clk each from one warp, which is why two warps per operand issue them: profiles/r1_gather_modes.md).
+    // gather_mode 1 (SIFT_GATHER_MODE=1) = every thread copies 16-byte pieces of the listed rows with cp.async,
+    // applying the 128-byte swizzle by hand (chunk ^= row & 7) so that the landed image is what a tiled box would
+    // have written; completion is signalled by cp.async.mbarrier.arrive.  Both are parity-tested.
     const bool is_k = warp < 4;
     const int ptid = is_k ? (int)threadIdx.x - 64 : (int)threadIdx.x - kFirstVWarp * 32;
     const int n_stages = is_k ? S::kKStages : S::kVStages;
@@ -277,7 +298,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       auto emit = [&](bool gather, int src, int act, bool last) {
         // src: gather -> index of the first cross entry of the group; tiled -> first key row
         const uint32_t full = bar(b_full + st), dst = ring + st * S::kTileBytes;
-        if (gather && p.gather_mode == 0) {
+        if (gather && p.gather_mode == 1) {
           const int32_t* ip = p.cross_idx + (int64_t)it.h * p.cross_cap + src + rr;
           int rows[PCH];
 #pragma unroll
@@ -394,8 +415,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       // MMA operand is built from uniform counters (kst, vst, j) and constants.
 #define SIFT_ISSUE_PV(q, ACC)                                                                                    \
   if (elect_one()) {                                                                                             \
-    _Pragma("unroll") for (int k = 0; k < kBN / 16; ++k)                                                         \
-        umma_ts(kTmemO + q * 128, kTmemS + q * 128 + k * 8, v_desc<HD>(vt, k), idesc_pv, (ACC) | (k > 0));      \
+    issue_pv<HD, q, ACC>(tz, vt, idesc_pv);                                                                      \
     umma_commit(bar(S::bODone + q));                                                                             \
   }                                                                                                              \
   __syncwarp();
@@ -406,6 +426,15 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     tc_fence_after();                                                                                            \
     if (fresh & (1 << q)) { SIFT_ISSUE_PV(q, 0) } else { SIFT_ISSUE_PV(q, 1) }                                   \
     fresh &= ~(1 << q);                                                                                          \
+  }
+#define SIFT_QK_STEP(q)                                                                                          \
+  SIFT_PV_STEP(q)                                                                                                \
+  if (act & (1 << q)) {                                                                                          \
+    if (elect_one()) {                                                                                           \
+      issue_qk<HD, q>(tz, q_smem + q * S::kTileBytes, kt, idesc_qk);                                             \
+      umma_commit(bar(S::bSFull + q));                                                                           \
+    }                                                                                                            \
+    __syncwarp();                                                                                                \
   }
       int pending = 0, fresh = (1 << kNQ) - 1;   // fresh bit q: the next P V of tile q overwrites O instead of accumulating
       bool last = false;
@@ -418,19 +447,8 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         if (j > 0) mbar_wait(bar(S::bVFull + vst), vph, 203);
         CFENCE();   // cp.async-gathered tiles were written through the generic proxy
         tc_fence_after();
-#pragma unroll
-        for (int q = 0; q < kNQ; ++q) {
-          SIFT_PV_STEP(q)
-          if (act & (1 << q)) {
-            if (elect_one()) {
-#pragma unroll
-              for (int k = 0; k < HD / 16; ++k)
-                umma_ss(kTmemS + q * 128, kmajor_desc<HD>(q_smem + q * S::kTileBytes, k), kmajor_desc<HD>(kt, k), idesc_qk, k > 0);
-              umma_commit(bar(S::bSFull + q));
-            }
-            __syncwarp();
-          }
-        }
+        SIFT_QK_STEP(0)
+        if constexpr (kNQ == 2) { SIFT_QK_STEP(1) }
         if (elect_one()) {
           if (j > 0) umma_commit(bar(S::bVEmpty + vst));
           umma_commit(bar(S::bKEmpty + kst));
@@ -447,26 +465,38 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         mbar_wait(bar(S::bVFull + vst), vph, 203);
         CFENCE();
         tc_fence_after();
-#pragma unroll
-        for (int q = 0; q < kNQ; ++q) { SIFT_PV_STEP(q) }
+        SIFT_PV_STEP(0)
+        if constexpr (kNQ == 2) { SIFT_PV_STEP(1) }
         if (elect_one()) umma_commit(bar(S::bVEmpty + vst));
         __syncwarp();
         if (++vst == S::kVStages) { vst = 0; vph ^= 1; }
       }
+#undef SIFT_QK_STEP
 #undef SIFT_PV_STEP
 #undef SIFT_ISSUE_PV
     }
   } else if (warp >= 4 && warp < kFirstVWarp) {
     // ======================================= softmax warpgroups =======================================
+    // Both warpgroups work on the SAME query tile at a time, each on one half of the 128 key columns of S (thread =
+    // one row x 64 columns), and alternate between the two tiles of the item.  A tile's softmax latency (S-full ->
+    // P-full) is what the tensor pipe has to hide behind the other tile's P V + Q K^T; with one warpgroup per tile
+    // that latency was ~1600 clk against 1024 clk of MMA (a lone warp per sub-partition cannot issue 128 ex2 in less
+    // than 1024 clk).  Splitting the columns halves it at the price of one row-max exchange through shared memory
+    // per step (named barrier 1, 256 threads); the row sums stay private per half until the epilogue.
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
-    const int q = (warp - 4) >> 2;
-    const int r = threadIdx.x - 128 - q * 128;             // row inside the query tile = TMEM lane
+    const int wg = (warp - 4) >> 2;                        // column half
+    const int r = ((warp & 3) << 5) | lane;                // row inside the query tile = TMEM lane
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
-    const uint32_t s_addr = tmem_base + lane_addr + q * 128;
-    const uint32_t o_addr = tmem_base + lane_addr + 256 + q * 128;
+    float* xch = reinterpret_cast<float*>(sgen + S::kXchgOff);   // [2 parities][2 halves][128 rows]
     const float sl = p.scale_log2;
-    uint32_t sph = 0;
-    uint32_t pv_cnt = 0;
+    uint32_t sph[kNQ] = {0, 0}, pv_cnt[kNQ] = {0, 0}, xpar = 0;
+    auto exchange = [&](float mine) -> float {            // returns the partner half's value for the same row
+      xch[(xpar * 2 + wg) * 128 + r] = mine;
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      const float other = xch[(xpar * 2 + (wg ^ 1)) * 128 + r];
+      xpar ^= 1;
+      return other;
+    };
     for (int it_n = 0;; ++it_n) {
       const int slot = it_n & 1;
       mbar_wait(bar(S::bItemFull + slot), (it_n >> 1) & 1, 300);
@@ -474,69 +504,51 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       mbar_arrive(bar(S::bItemEmpty + slot));
       if (code < 0) break;
       const Item it = load_item(p, code);
-      if (it.rows[q] <= 0) continue;
-      const int ngroups = it.is_dense ? 0 : (it.cp + kBN - 1) / kBN;
-      const int nsteps = it.is_dense ? dense_steps(it.row0[q], it.rows[q]) : ngroups + it.lcnt[q];
-      bool last_is_diag = false;
-      if (!it.is_dense && it.lcnt[q] > 0)
-        last_is_diag = p.local_idx[(int64_t)it.h * p.local_cap + it.lptr[q] + it.lcnt[q] - 1] == it.tile_id[q];
-      float m = -INFINITY, l = 0.f;
-      for (int e = 0; e < nsteps; ++e) {
-        int n_valid = kBN, kdelta = 0;
-        bool causal = false;
-        if (it.is_dense) {
-          kdelta = e * kBN - it.row0[q];
-          causal = kdelta + kBN - 1 > 0;
-        } else if (e < ngroups) {
-          n_valid = min(kBN, it.cp - e * kBN);
-        } else {
-          n_valid = min(kBN, p.tile);
-          causal = last_is_diag && (e == nsteps - 1);
-        }
-        mbar_wait(bar(S::bSFull + q), sph, 301);
-        sph ^= 1;
+      float m[kNQ] = {-INFINITY, -INFINITY}, l[kNQ] = {0.f, 0.f};
+      int done[kNQ] = {0, 0};                              // steps of tile t processed in this item
+      // one step of tile T: columns [wg*64, wg*64+64) of S -> P
+      auto step = [&](auto TC, int n_valid, bool causal, int kdelta) {
+        constexpr int T = decltype(TC)::value;
+        mbar_wait(bar(S::bSFull + T), sph[T], 301);
+        sph[T] ^= 1;
         tc_fence_after();
-#if defined(SIFT_ABL) && SIFT_ABL == 2
-        tc_fence_before(); mbar_arrive(bar(S::bPFull + q)); ++pv_cnt; l = 1.f; m = 0.f; continue;
-#endif
-        float s[kBN];
+        const uint32_t s_addr = lane_addr + T * 128 + wg * 64;
+        float s[64];
         {
-          uint32_t raw0[32], raw1[32], raw2[32], raw3[32];
-          tmem_ld32(s_addr + 0, raw0);
+          uint32_t raw0[32], raw1[32];
+          tmem_ld32(s_addr, raw0);
           tmem_ld32(s_addr + 32, raw1);
-          tmem_ld32(s_addr + 64, raw2);
-          tmem_ld32(s_addr + 96, raw3);
           tmem_wait_ld();
 #pragma unroll
-          for (int c = 0; c < 32; ++c) {
-            s[c] = __uint_as_float(raw0[c]); s[32 + c] = __uint_as_float(raw1[c]);
-            s[64 + c] = __uint_as_float(raw2[c]); s[96 + c] = __uint_as_float(raw3[c]);
-          }
+          for (int c = 0; c < 32; ++c) { s[c] = __uint_as_float(raw0[c]); s[32 + c] = __uint_as_float(raw1[c]); }
         }
         if (causal || n_valid < kBN) {
-          const int lim = causal ? min(n_valid, r - kdelta + 1) : n_valid;   // columns [0, lim) are allowed
+          // columns [0, lim) of the tile are allowed; this thread holds columns wg*64 ..
+          const int lim = (causal ? min(n_valid, r - kdelta + 1) : n_valid) - wg * 64;
 #pragma unroll
-          for (int c = 0; c < kBN; ++c) s[c] = (c < lim) ? s[c] : -INFINITY;
+          for (int c = 0; c < 64; ++c) s[c] = (c < lim) ? s[c] : -INFINITY;
         }
         float mx4[4] = {s[0], s[1], s[2], s[3]};                  // four independent chains
 #pragma unroll
-        for (int c = 4; c < kBN; c += 4) {
+        for (int c = 4; c < 64; c += 4) {
           mx4[0] = fmaxf(mx4[0], s[c]); mx4[1] = fmaxf(mx4[1], s[c + 1]);
           mx4[2] = fmaxf(mx4[2], s[c + 2]); mx4[3] = fmaxf(mx4[3], s[c + 3]);
         }
-        const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
-        const float m_new = fmaxf(m, mx);
-        const bool need = (m_new - m) * sl > kRescaleThreshold;   // (-inf) - (-inf) = NaN -> false
+        float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
+        mx = fmaxf(mx, exchange(mx));                              // row max over all 128 columns
+        const float m_new = fmaxf(m[T], mx);
+        const bool need = (m_new - m[T]) * sl > kRescaleThreshold;   // (-inf) - (-inf) = NaN -> false
         if (__any_sync(0xffffffffu, need)) {
-          const float alpha = need ? ex2((m - m_new) * sl) : 1.f;
-          l *= alpha;
-          if (need) m = m_new;
-          if (e > 0) {
-            // O of this tile must hold every P*V issued so far before it is rescaled
-            mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 302);
+          const float alpha = need ? ex2((m[T] - m_new) * sl) : 1.f;
+          l[T] *= alpha;
+          if (need) m[T] = m_new;
+          if (done[T] > 0) {
+            // O of this tile must hold every P*V issued so far before it is rescaled (this half's columns)
+            mbar_wait(bar(S::bODone + T), (pv_cnt[T] - 1) & 1, 302);
             tc_fence_after();
+            const uint32_t o_addr = lane_addr + 256 + T * 128 + wg * (HD / 2);
 #pragma unroll
-            for (int c = 0; c < HD / 32; ++c) {
+            for (int c = 0; c < HD / 64; ++c) {
               uint32_t o[32];
               tmem_ld32(o_addr + c * 32, o);
               tmem_wait_ld();
@@ -546,10 +558,10 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             }
           }
         }
-        const float neg_m = (m == -INFINITY) ? 0.f : -m * sl;
+        const float neg_m = (m[T] == -INFINITY) ? 0.f : -m[T] * sl;
         float sum0 = 0.f, sum1 = 0.f;
 #pragma unroll
-        for (int c = 0; c < kBN / 32; ++c) {
+        for (int c = 0; c < 2; ++c) {
           uint32_t pk[16];
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
@@ -567,48 +579,91 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           // P (bf16) overwrites the first 64 columns of S: 16 packed columns per 32 keys
           asm volatile(
               "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-              ::"r"(s_addr + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
-                "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
-                "r"(pk[15]) : "memory");
+              ::"r"(lane_addr + T * 128 + wg * 32 + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]),
+                "r"(pk[5]), "r"(pk[6]), "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]),
+                "r"(pk[13]), "r"(pk[14]), "r"(pk[15]) : "memory");
         }
-        l += sum0 + sum1;
+        l[T] += sum0 + sum1;
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(bar(S::bPFull + q));
-        ++pv_cnt;
+        mbar_arrive(bar(S::bPFull + T));
+        ++pv_cnt[T];
+        ++done[T];
+      };
+      using T0 = std::integral_constant<int, 0>;
+      using T1 = std::integral_constant<int, 1>;
+      // ---- the steps, in exactly the order the producers emit them (tile 0 before tile 1 inside a step)
+      int nsteps[kNQ];
+      if (it.is_dense) {
+        nsteps[0] = dense_steps(it.row0[0], it.rows[0]);
+        nsteps[1] = dense_steps(it.row0[1], it.rows[1]);
+        const int total = max(nsteps[0], nsteps[1]);
+        for (int j = 0; j < total; ++j) {
+          if (j < nsteps[0]) { const int kd = j * kBN - it.row0[0]; step(T0{}, kBN, kd + kBN - 1 > 0, kd); }
+          if (j < nsteps[1]) { const int kd = j * kBN - it.row0[1]; step(T1{}, kBN, kd + kBN - 1 > 0, kd); }
+        }
+      } else {
+        const int ngroups = (it.cp + kBN - 1) / kBN;
+        nsteps[0] = it.rows[0] > 0 ? ngroups + it.lcnt[0] : 0;
+        nsteps[1] = it.rows[1] > 0 ? ngroups + it.lcnt[1] : 0;
+        for (int g = 0; g < ngroups; ++g) {
+          const int nv = min(kBN, it.cp - g * kBN);
+          if (it.rows[0] > 0) step(T0{}, nv, false, 0);
+          if (it.rows[1] > 0) step(T1{}, nv, false, 0);
+        }
+        const int32_t* lidx = p.local_idx + (int64_t)it.h * p.local_cap;
+        const int nv = min(kBN, p.tile);
+        int pos0 = 0, pos1 = 0;
+        while (true) {
+          const int cur0 = pos0 < it.lcnt[0] ? lidx[it.lptr[0] + pos0] : 0x7fffffff;
+          const int cur1 = pos1 < it.lcnt[1] ? lidx[it.lptr[1] + pos1] : 0x7fffffff;
+          const int t = min(cur0, cur1);
+          if (t == 0x7fffffff) break;
+          if (cur0 == t) { step(T0{}, nv, t == it.tile_id[0], 0); ++pos0; }   // the diagonal tile is causally masked
+          if (cur1 == t) { step(T1{}, nv, t == it.tile_id[1], 0); ++pos1; }
+        }
       }
-      // ---- epilogue: O / l -> bf16, LSE
-      const int64_t grow = (int64_t)it.row0[q] + r;
-      const bool row_ok = r < it.rows[q];
-      __nv_bfloat16* orow = p.o + grow * p.o_row_stride + (int64_t)it.h * HD;
-      if (nsteps > 0) {
-        mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 303);
-        tc_fence_after();
-        const float inv = l > 0.f ? 1.f / l : 0.f;
+      // ---- epilogue: O / l -> bf16 (this half's head-dim columns), LSE
+      auto finish = [&](auto TC) {
+        constexpr int T = decltype(TC)::value;
+        if (it.rows[T] <= 0) return;
+        const int64_t grow = (int64_t)it.row0[T] + r;
+        const bool row_ok = r < it.rows[T];
+        __nv_bfloat16* orow = p.o + grow * p.o_row_stride + (int64_t)it.h * HD + wg * (HD / 2);
+        float lt = 0.f;
+        if (nsteps[T] > 0) {
+          lt = l[T] + exchange(l[T]);
+          mbar_wait(bar(S::bODone + T), (pv_cnt[T] - 1) & 1, 303);
+          tc_fence_after();
+          const float inv = lt > 0.f ? 1.f / lt : 0.f;
+          const uint32_t o_addr = lane_addr + 256 + T * 128 + wg * (HD / 2);
 #pragma unroll
-        for (int c = 0; c < HD / 32; ++c) {
-          uint32_t o[32];
-          tmem_ld32(o_addr + c * 32, o);
-          tmem_wait_ld();
-          if (row_ok) {
+          for (int c = 0; c < HD / 64; ++c) {
+            uint32_t o[32];
+            tmem_ld32(o_addr + c * 32, o);
+            tmem_wait_ld();
+            if (row_ok) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              uint4 w;
-              w.x = pack_bf16x2(__uint_as_float(o[8 * i + 0]) * inv, __uint_as_float(o[8 * i + 1]) * inv);
-              w.y = pack_bf16x2(__uint_as_float(o[8 * i + 2]) * inv, __uint_as_float(o[8 * i + 3]) * inv);
-              w.z = pack_bf16x2(__uint_as_float(o[8 * i + 4]) * inv, __uint_as_float(o[8 * i + 5]) * inv);
-              w.w = pack_bf16x2(__uint_as_float(o[8 * i + 6]) * inv, __uint_as_float(o[8 * i + 7]) * inv);
-              *reinterpret_cast<uint4*>(orow + c * 32 + i * 8) = w;
+              for (int i = 0; i < 4; ++i) {
+                uint4 w;
+                w.x = pack_bf16x2(__uint_as_float(o[8 * i + 0]) * inv, __uint_as_float(o[8 * i + 1]) * inv);
+                w.y = pack_bf16x2(__uint_as_float(o[8 * i + 2]) * inv, __uint_as_float(o[8 * i + 3]) * inv);
+                w.z = pack_bf16x2(__uint_as_float(o[8 * i + 4]) * inv, __uint_as_float(o[8 * i + 5]) * inv);
+                w.w = pack_bf16x2(__uint_as_float(o[8 * i + 6]) * inv, __uint_as_float(o[8 * i + 7]) * inv);
+                *reinterpret_cast<uint4*>(orow + c * 32 + i * 8) = w;
+              }
             }
           }
-        }
-        tc_fence_before();
-      } else if (row_ok) {
+          tc_fence_before();
+        } else if (row_ok) {
 #pragma unroll
-        for (int i = 0; i < HD / 8; ++i) *reinterpret_cast<uint4*>(orow + i * 8) = make_uint4(0, 0, 0, 0);
-      }
-      if (row_ok && p.lse != nullptr)
-        p.lse[(int64_t)it.h * p.n_tokens + grow] = (l > 0.f) ? (m * sl + log2f(l)) * 0.6931471805599453f : -INFINITY;
+          for (int i = 0; i < HD / 16; ++i) *reinterpret_cast<uint4*>(orow + i * 8) = make_uint4(0, 0, 0, 0);
+        }
+        if (row_ok && wg == 0 && p.lse != nullptr)
+          p.lse[(int64_t)it.h * p.n_tokens + grow] = (lt > 0.f) ? (m[T] * sl + log2f(lt)) * 0.6931471805599453f : -INFINITY;
+      };
+      finish(T0{});
+      finish(T1{});
     }
   } else {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));   // idle warps only donate registers
@@ -671,7 +726,7 @@ static int launch_attention(AttnParams& p, const void* Q, const void* K, const v
   int rc;
   p.k_ptr = static_cast<const char*>(K); p.v_ptr = static_cast<const char*>(V);
   p.k_row_bytes = ks * 2; p.v_row_bytes = vs * 2;
-  { const char* e = getenv("SIFT_GATHER_MODE"); p.gather_mode = (e && e[0] == '1') ? 1 : 0; }  // 1 = TMA gather4 (comparison)
+  { const char* e = getenv("SIFT_GATHER_MODE"); p.gather_mode = (e && e[0] == '1') ? 1 : 0; }  // 1 = cp.async row gather
   const int64_t n = p.n_tokens;
   if ((rc = make_map(&tq, Q, n, (int64_t)p.n_q_heads * HD, qs, kBM))) return rc;
   if ((rc = make_map(&tk, K, n, (int64_t)p.n_kv_heads * HD, ks, kBN))) return rc;

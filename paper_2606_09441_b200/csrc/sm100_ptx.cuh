@@ -121,6 +121,24 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
       ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accum) : "memory");
 }
 
+// Same two forms with the TMEM addresses given as (uniform run-time base) + (compile-time offset): the adds sit next
+// to the MMA, so the addresses are rebuilt in uniform registers instead of being hoisted into vector registers and
+// moved back with R2UR on every issue.
+template <uint32_t DOFF>
+__device__ __forceinline__ void umma_ss_off(uint32_t tbase, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b32 d;\n\tsetp.ne.b32 p, %4, 0;\n\tadd.u32 d, %0, %5;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [d], %1, %2, %3, p;\n\t}"
+      ::"r"(tbase), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accum), "n"(DOFF) : "memory");
+}
+template <uint32_t DOFF, uint32_t AOFF>
+__device__ __forceinline__ void umma_ts_off(uint32_t tbase, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b32 d, a;\n\tsetp.ne.b32 p, %3, 0;\n\tadd.u32 d, %0, %4;\n\tadd.u32 a, %0, %5;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [d], [a], %1, %2, p;\n\t}"
+      ::"r"(tbase), "l"(b_desc), "r"(idesc), "r"(accum), "n"(DOFF), "n"(AOFF) : "memory");
+}
+
 // Shared-memory matrix descriptor, 128-byte swizzle.  K-major: rows of 64 bf16 (128 B), 8-row groups SBO apart.
 // MN-major: 64 MN-elements (128 B) x 8 K-rows per atom, atoms LBO apart along MN and SBO apart along K.
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {

@@ -77,6 +77,18 @@ def test_cross_gather_only():
     _report("cross+diag", gu.attention_errors(w, 0, o, lse, [0, 1], range(w.shape.n_tokens)))
 
 
+@pytest.mark.parametrize("case", [
+    dict(n_q_heads=2, n_kv_heads=2, head_dim=128, doc_lens=(384, 256, 700), query_len=40, tile=128, p_cross=0.4),
+    dict(n_q_heads=2, n_kv_heads=1, head_dim=64, doc_lens=(256, 300, 129), query_len=0, tile=64, p_cross=0.7),
+])
+def test_cross_gather_cp_async_mode(case, monkeypatch):
+    """The alternative row-gather path (SIFT_GATHER_MODE=1: swizzled cp.async instead of TMA gather4)."""
+    monkeypatch.setenv("SIFT_GATHER_MODE", "1")
+    w = wl.custom("cross-cpasync", seed=23, **case)
+    _, _, o, lse = gu.run_sift(w)
+    _report(f"cp.async gather {case}", gu.attention_errors(w, 0, o, lse, range(w.shape.n_q_heads), range(w.shape.n_tokens)))
+
+
 def test_empty_rows_A13():
     w = wl.custom("empty", n_q_heads=1, head_dim=64, doc_lens=(200, 100), query_len=30, tile=64, p_loc=-1.0,
                   p_cross=-1.0, diag_set=False, seed=5)
@@ -121,6 +133,24 @@ def test_config_sampled_rows(cfg, heads):
     _, _, o, lse = gu.run_sift(w)
     assert torch.isfinite(o.float()).all()
     _report(cfg, gu.attention_errors(w, 0, o, lse, heads, gu.sample_rows(w)))
+
+
+def test_full_stack_layers_and_reorder_sampled():
+    """C5 shape (4 of its 32 layers to bound host memory): one decode call for all layers, then per-layer attention;
+    a re-ordered prompt (vectors travel with their document) is checked against the oracle on the permuted inputs."""
+    w = wl.config_full_stack(n_layers=4)
+    shape, md = gu.decode_on_gpu(w)
+    for layer in (0, 3):
+        q, k, v = (t.cuda() for t in w.qkv(layer))
+        o, lse = api.sift_prefill_attention(shape, layer, q, k, v, md)
+        torch.cuda.synchronize()
+        _report(f"C5 layer {layer}", gu.attention_errors(w, layer, o, lse, [1, 22], gu.sample_rows(w, n_per_seg=2)))
+    w2 = w.reorder(wl.stack_orderings(w)[1])
+    shape2, md2 = gu.decode_on_gpu(w2)
+    q, k, v = (t.cuda() for t in w2.qkv(2))
+    o, lse = api.sift_prefill_attention(shape2, 2, q, k, v, md2)
+    torch.cuda.synchronize()
+    _report("C5 reordered layer 2", gu.attention_errors(w2, 2, o, lse, [7], gu.sample_rows(w2, n_per_seg=2)))
 
 
 def test_repeat_calls_share_metadata():
