@@ -38,6 +38,10 @@ constexpr int kFirstVWarp = 4 + 4 * kNQ;
 constexpr int kProducerThreads = 64;              // per operand
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 with a stale max
 constexpr uint32_t kTmemCols = 512;
+#ifndef SIFT_EXP_EMU_MASK
+#define SIFT_EXP_EMU_MASK 0x0
+#endif
+constexpr int kExpEmuMask = SIFT_EXP_EMU_MASK;   // bit j: pairs with (index & 3) == j compute 2^x by polynomial instead of MUFU.EX2
 
 constexpr int kRegsEntry = (kNQ == 2) ? 128 : 168;               // what __launch_bounds__(kNumThreads, 1) yields
 constexpr int kRegsOther = 48;                                   // non-softmax warps after setmaxnreg.dec
@@ -201,7 +205,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     for (int i = 0; i < S::kVStages; ++i) { mbar_init(bar(S::bVFull + i), kProducerThreads); mbar_init(bar(S::bVEmpty + i), 1); }
     for (int q = 0; q < kNQ; ++q) {
       mbar_init(bar(S::bSFull + q), 1);
-      mbar_init(bar(S::bPFull + q), 256);   // both column halves
+      mbar_init(bar(S::bPFull + q), 128);
       mbar_init(bar(S::bODone + q), 1);
     }
     for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 5 + 128 * kNQ); }
@@ -477,78 +481,89 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     }
   } else if (warp >= 4 && warp < kFirstVWarp) {
     // ======================================= softmax warpgroups =======================================
-    // Both warpgroups work on the SAME query tile at a time, each on one half of the 128 key columns of S (thread =
-    // one row x 64 columns), and alternate between the two tiles of the item.  A tile's softmax latency (S-full ->
-    // P-full) is what the tensor pipe has to hide behind the other tile's P V + Q K^T; with one warpgroup per tile
-    // that latency was ~1600 clk against 1024 clk of MMA (a lone warp per sub-partition cannot issue 128 ex2 in less
-    // than 1024 clk).  Splitting the columns halves it at the price of one row-max exchange through shared memory
-    // per step (named barrier 1, 256 threads); the row sums stay private per half until the epilogue.
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
-    const int wg = (warp - 4) >> 2;                        // column half
-    const int r = ((warp & 3) << 5) | lane;                // row inside the query tile = TMEM lane
+    // One warpgroup per query tile, one row per thread.  ONE copy of the code for both warpgroups (two instantiations
+    // measured 7% slower: the loop body is ~10 KB of SASS and both copies would compete for the instruction caches of
+    // every sub-partition); the item fields of "my" tile are picked with selects, not indexed (no local memory).
+    {
+    const int q = (warp - 4) >> 2;
+    const int r = (int)threadIdx.x - 128 - q * 128;        // row inside the query tile = TMEM lane
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
-    float* xch = reinterpret_cast<float*>(sgen + S::kXchgOff);   // [2 parities][2 halves][128 rows]
+    const uint32_t s_addr = lane_addr + q * 128;
+    const uint32_t o_addr = lane_addr + 256 + q * 128;
     const float sl = p.scale_log2;
-    uint32_t sph[kNQ] = {0, 0}, pv_cnt[kNQ] = {0, 0}, xpar = 0;
-    auto exchange = [&](float mine) -> float {            // returns the partner half's value for the same row
-      xch[(xpar * 2 + wg) * 128 + r] = mine;
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      const float other = xch[(xpar * 2 + (wg ^ 1)) * 128 + r];
-      xpar ^= 1;
-      return other;
-    };
+    const int tile_lim = min(kBN, p.tile);
+    uint32_t sph = 0;
+    uint32_t pv_cnt = 0;
     for (int it_n = 0;; ++it_n) {
       const int slot = it_n & 1;
       mbar_wait(bar(S::bItemFull + slot), (it_n >> 1) & 1, 300);
       const int code = info[1 + slot];
       mbar_arrive(bar(S::bItemEmpty + slot));
       if (code < 0) break;
-      const Item it = load_item(p, code);
-      float m[kNQ] = {-INFINITY, -INFINITY}, l[kNQ] = {0.f, 0.f};
-      int done[kNQ] = {0, 0};                              // steps of tile t processed in this item
-      // one step of tile T: columns [wg*64, wg*64+64) of S -> P
-      auto step = [&](auto TC, int n_valid, bool causal, int kdelta) {
-        constexpr int T = decltype(TC)::value;
-        mbar_wait(bar(S::bSFull + T), sph[T], 301);
-        sph[T] ^= 1;
+      int row0, rows, h, ngroups, nsteps, diag_step, lim;
+      {
+        const Item it = load_item(p, code);
+        row0 = q ? it.row0[1] : it.row0[0]; rows = q ? it.rows[1] : it.rows[0]; h = it.h;
+        const int lcnt = q ? it.lcnt[1] : it.lcnt[0], lptr = q ? it.lptr[1] : it.lptr[0];
+        const int tile_id = q ? it.tile_id[1] : it.tile_id[0];
+        if (rows <= 0) continue;
+        ngroups = it.is_dense ? 0 : (it.cp + kBN - 1) / kBN;
+        nsteps = it.is_dense ? dense_steps(row0, rows) : ngroups + lcnt;
+        diag_step = -1;                                   // the step (if any) that is the causally masked diagonal tile
+        if (!it.is_dense && lcnt > 0 && p.local_idx[(int64_t)h * p.local_cap + lptr + lcnt - 1] == tile_id)
+          diag_step = nsteps - 1;
+        // columns [0, lim) of the current step are allowed for this row; lim drops by kBN per step in the cross
+        // phase (ragged last group) and in DENSE items (causal frontier)
+        lim = it.is_dense ? row0 + r + 1 : it.cp;
+        if (it.is_dense) ngroups = nsteps;                // "frontier" steps: all of them
+      }
+      float m = -INFINITY, l = 0.f;
+      for (int e = 0; e < nsteps; ++e, lim -= kBN) {
+        const int cur_lim = (e < ngroups) ? lim : (e == diag_step ? min(tile_lim, r + 1) : tile_lim);
+        mbar_wait(bar(S::bSFull + q), sph, 301);
+        sph ^= 1;
         tc_fence_after();
-        const uint32_t s_addr = lane_addr + T * 128 + wg * 64;
-        float s[64];
+#if defined(SIFT_ABL) && SIFT_ABL == 2
+        tc_fence_before(); mbar_arrive(bar(S::bPFull + q)); ++pv_cnt; l = 1.f; m = 0.f; continue;
+#endif
+        float s[kBN];
         {
-          uint32_t raw0[32], raw1[32];
-          tmem_ld32(s_addr, raw0);
+          uint32_t raw0[32], raw1[32], raw2[32], raw3[32];
+          tmem_ld32(s_addr + 0, raw0);
           tmem_ld32(s_addr + 32, raw1);
+          tmem_ld32(s_addr + 64, raw2);
+          tmem_ld32(s_addr + 96, raw3);
           tmem_wait_ld();
 #pragma unroll
-          for (int c = 0; c < 32; ++c) { s[c] = __uint_as_float(raw0[c]); s[32 + c] = __uint_as_float(raw1[c]); }
+          for (int c = 0; c < 32; ++c) {
+            s[c] = __uint_as_float(raw0[c]); s[32 + c] = __uint_as_float(raw1[c]);
+            s[64 + c] = __uint_as_float(raw2[c]); s[96 + c] = __uint_as_float(raw3[c]);
+          }
         }
-        if (causal || n_valid < kBN) {
-          // columns [0, lim) of the tile are allowed; this thread holds columns wg*64 ..
-          const int lim = (causal ? min(n_valid, r - kdelta + 1) : n_valid) - wg * 64;
+        if (__any_sync(0xffffffffu, cur_lim < kBN)) {
 #pragma unroll
-          for (int c = 0; c < 64; ++c) s[c] = (c < lim) ? s[c] : -INFINITY;
+          for (int c = 0; c < kBN; ++c) s[c] = (c < cur_lim) ? s[c] : -INFINITY;
         }
         float mx4[4] = {s[0], s[1], s[2], s[3]};                  // four independent chains
 #pragma unroll
-        for (int c = 4; c < 64; c += 4) {
+        for (int c = 4; c < kBN; c += 4) {
           mx4[0] = fmaxf(mx4[0], s[c]); mx4[1] = fmaxf(mx4[1], s[c + 1]);
           mx4[2] = fmaxf(mx4[2], s[c + 2]); mx4[3] = fmaxf(mx4[3], s[c + 3]);
         }
-        float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
-        mx = fmaxf(mx, exchange(mx));                              // row max over all 128 columns
-        const float m_new = fmaxf(m[T], mx);
-        const bool need = (m_new - m[T]) * sl > kRescaleThreshold;   // (-inf) - (-inf) = NaN -> false
+        const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
+        const float m_new = fmaxf(m, mx);
+        const bool need = (m_new - m) * sl > kRescaleThreshold;   // (-inf) - (-inf) = NaN -> false
         if (__any_sync(0xffffffffu, need)) {
-          const float alpha = need ? ex2((m[T] - m_new) * sl) : 1.f;
-          l[T] *= alpha;
-          if (need) m[T] = m_new;
-          if (done[T] > 0) {
-            // O of this tile must hold every P*V issued so far before it is rescaled (this half's columns)
-            mbar_wait(bar(S::bODone + T), (pv_cnt[T] - 1) & 1, 302);
+          const float alpha = need ? ex2((m - m_new) * sl) : 1.f;
+          l *= alpha;
+          if (need) m = m_new;
+          if (e > 0) {
+            // O of this tile must hold every P*V issued so far before it is rescaled
+            mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 302);
             tc_fence_after();
-            const uint32_t o_addr = lane_addr + 256 + T * 128 + wg * (HD / 2);
 #pragma unroll
-            for (int c = 0; c < HD / 64; ++c) {
+            for (int c = 0; c < HD / 32; ++c) {
               uint32_t o[32];
               tmem_ld32(o_addr + c * 32, o);
               tmem_wait_ld();
@@ -558,112 +573,76 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             }
           }
         }
-        const float neg_m = (m[T] == -INFINITY) ? 0.f : -m[T] * sl;
-        float sum0 = 0.f, sum1 = 0.f;
+        const float neg_m = (m == -INFINITY) ? 0.f : -m * sl;
+        float2 sum_a = make_float2(0.f, 0.f), sum_b = make_float2(0.f, 0.f);
+        const float2 sl2 = make_float2(sl, sl), nm2 = make_float2(neg_m, neg_m);
 #pragma unroll
-        for (int c = 0; c < 2; ++c) {
+        for (int c = 0; c < kBN / 32; ++c) {
           uint32_t pk[16];
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
+            const float2 x = fma2(make_float2(s[c * 32 + 2 * i], s[c * 32 + 2 * i + 1]), sl2, nm2);
+            float2 pr;
+            if ((kExpEmuMask >> (i & 3)) & 1) {
+              pr = ex2_poly2(x);                 // this pair on the FMA pipe: the MUFU is the co-bottleneck (DESIGN 5.2)
+            } else {
 #if defined(SIFT_ABL) && SIFT_ABL == 1
-            const float p0 = fmaf(s[c * 32 + 2 * i], sl, neg_m);
-            const float p1 = fmaf(s[c * 32 + 2 * i + 1], sl, neg_m);
+              pr = x;
 #else
-            const float p0 = ex2(fmaf(s[c * 32 + 2 * i], sl, neg_m));
-            const float p1 = ex2(fmaf(s[c * 32 + 2 * i + 1], sl, neg_m));
+              pr = make_float2(ex2(x.x), ex2(x.y));
 #endif
-            sum0 += p0;
-            sum1 += p1;
-            pk[i] = pack_bf16x2(p0, p1);
+            }
+            if (i & 1) sum_b = add2(sum_b, pr); else sum_a = add2(sum_a, pr);
+            pk[i] = pack_bf16x2(pr.x, pr.y);
           }
           // P (bf16) overwrites the first 64 columns of S: 16 packed columns per 32 keys
           asm volatile(
               "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-              ::"r"(lane_addr + T * 128 + wg * 32 + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]),
-                "r"(pk[5]), "r"(pk[6]), "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]),
-                "r"(pk[13]), "r"(pk[14]), "r"(pk[15]) : "memory");
+              ::"r"(s_addr + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
+                "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
+                "r"(pk[15]) : "memory");
         }
-        l[T] += sum0 + sum1;
+        const float2 sum2 = add2(sum_a, sum_b);
+        const float sum0 = sum2.x, sum1 = sum2.y;
+        l += sum0 + sum1;
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(bar(S::bPFull + T));
-        ++pv_cnt[T];
-        ++done[T];
-      };
-      using T0 = std::integral_constant<int, 0>;
-      using T1 = std::integral_constant<int, 1>;
-      // ---- the steps, in exactly the order the producers emit them (tile 0 before tile 1 inside a step)
-      int nsteps[kNQ];
-      if (it.is_dense) {
-        nsteps[0] = dense_steps(it.row0[0], it.rows[0]);
-        nsteps[1] = dense_steps(it.row0[1], it.rows[1]);
-        const int total = max(nsteps[0], nsteps[1]);
-        for (int j = 0; j < total; ++j) {
-          if (j < nsteps[0]) { const int kd = j * kBN - it.row0[0]; step(T0{}, kBN, kd + kBN - 1 > 0, kd); }
-          if (j < nsteps[1]) { const int kd = j * kBN - it.row0[1]; step(T1{}, kBN, kd + kBN - 1 > 0, kd); }
-        }
-      } else {
-        const int ngroups = (it.cp + kBN - 1) / kBN;
-        nsteps[0] = it.rows[0] > 0 ? ngroups + it.lcnt[0] : 0;
-        nsteps[1] = it.rows[1] > 0 ? ngroups + it.lcnt[1] : 0;
-        for (int g = 0; g < ngroups; ++g) {
-          const int nv = min(kBN, it.cp - g * kBN);
-          if (it.rows[0] > 0) step(T0{}, nv, false, 0);
-          if (it.rows[1] > 0) step(T1{}, nv, false, 0);
-        }
-        const int32_t* lidx = p.local_idx + (int64_t)it.h * p.local_cap;
-        const int nv = min(kBN, p.tile);
-        int pos0 = 0, pos1 = 0;
-        while (true) {
-          const int cur0 = pos0 < it.lcnt[0] ? lidx[it.lptr[0] + pos0] : 0x7fffffff;
-          const int cur1 = pos1 < it.lcnt[1] ? lidx[it.lptr[1] + pos1] : 0x7fffffff;
-          const int t = min(cur0, cur1);
-          if (t == 0x7fffffff) break;
-          if (cur0 == t) { step(T0{}, nv, t == it.tile_id[0], 0); ++pos0; }   // the diagonal tile is causally masked
-          if (cur1 == t) { step(T1{}, nv, t == it.tile_id[1], 0); ++pos1; }
-        }
+        mbar_arrive(bar(S::bPFull + q));
+        ++pv_cnt;
       }
-      // ---- epilogue: O / l -> bf16 (this half's head-dim columns), LSE
-      auto finish = [&](auto TC) {
-        constexpr int T = decltype(TC)::value;
-        if (it.rows[T] <= 0) return;
-        const int64_t grow = (int64_t)it.row0[T] + r;
-        const bool row_ok = r < it.rows[T];
-        __nv_bfloat16* orow = p.o + grow * p.o_row_stride + (int64_t)it.h * HD + wg * (HD / 2);
-        float lt = 0.f;
-        if (nsteps[T] > 0) {
-          lt = l[T] + exchange(l[T]);
-          mbar_wait(bar(S::bODone + T), (pv_cnt[T] - 1) & 1, 303);
-          tc_fence_after();
-          const float inv = lt > 0.f ? 1.f / lt : 0.f;
-          const uint32_t o_addr = lane_addr + 256 + T * 128 + wg * (HD / 2);
+      // ---- epilogue: O / l -> bf16, LSE
+      const int64_t grow = (int64_t)row0 + r;
+      const bool row_ok = r < rows;
+      __nv_bfloat16* orow = p.o + grow * p.o_row_stride + (int64_t)h * HD;
+      if (nsteps > 0) {
+        mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 303);
+        tc_fence_after();
+        const float inv = l > 0.f ? 1.f / l : 0.f;
 #pragma unroll
-          for (int c = 0; c < HD / 64; ++c) {
-            uint32_t o[32];
-            tmem_ld32(o_addr + c * 32, o);
-            tmem_wait_ld();
-            if (row_ok) {
+        for (int c = 0; c < HD / 32; ++c) {
+          uint32_t o[32];
+          tmem_ld32(o_addr + c * 32, o);
+          tmem_wait_ld();
+          if (row_ok) {
 #pragma unroll
-              for (int i = 0; i < 4; ++i) {
-                uint4 w;
-                w.x = pack_bf16x2(__uint_as_float(o[8 * i + 0]) * inv, __uint_as_float(o[8 * i + 1]) * inv);
-                w.y = pack_bf16x2(__uint_as_float(o[8 * i + 2]) * inv, __uint_as_float(o[8 * i + 3]) * inv);
-                w.z = pack_bf16x2(__uint_as_float(o[8 * i + 4]) * inv, __uint_as_float(o[8 * i + 5]) * inv);
-                w.w = pack_bf16x2(__uint_as_float(o[8 * i + 6]) * inv, __uint_as_float(o[8 * i + 7]) * inv);
-                *reinterpret_cast<uint4*>(orow + c * 32 + i * 8) = w;
-              }
+            for (int i = 0; i < 4; ++i) {
+              uint4 w;
+              w.x = pack_bf16x2(__uint_as_float(o[8 * i + 0]) * inv, __uint_as_float(o[8 * i + 1]) * inv);
+              w.y = pack_bf16x2(__uint_as_float(o[8 * i + 2]) * inv, __uint_as_float(o[8 * i + 3]) * inv);
+              w.z = pack_bf16x2(__uint_as_float(o[8 * i + 4]) * inv, __uint_as_float(o[8 * i + 5]) * inv);
+              w.w = pack_bf16x2(__uint_as_float(o[8 * i + 6]) * inv, __uint_as_float(o[8 * i + 7]) * inv);
+              *reinterpret_cast<uint4*>(orow + c * 32 + i * 8) = w;
             }
           }
-          tc_fence_before();
-        } else if (row_ok) {
-#pragma unroll
-          for (int i = 0; i < HD / 16; ++i) *reinterpret_cast<uint4*>(orow + i * 8) = make_uint4(0, 0, 0, 0);
         }
-        if (row_ok && wg == 0 && p.lse != nullptr)
-          p.lse[(int64_t)it.h * p.n_tokens + grow] = (lt > 0.f) ? (m[T] * sl + log2f(lt)) * 0.6931471805599453f : -INFINITY;
-      };
-      finish(T0{});
-      finish(T1{});
+        tc_fence_before();
+      } else if (row_ok) {
+#pragma unroll
+        for (int i = 0; i < HD / 8; ++i) *reinterpret_cast<uint4*>(orow + i * 8) = make_uint4(0, 0, 0, 0);
+      }
+      if (row_ok && p.lse != nullptr)
+        p.lse[(int64_t)h * p.n_tokens + grow] = (l > 0.f) ? (m * sl + log2f(l)) * 0.6931471805599453f : -INFINITY;
+    }
     }
   } else {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));   // idle warps only donate registers
