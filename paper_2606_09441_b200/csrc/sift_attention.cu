@@ -90,7 +90,7 @@ struct Smem {
   static constexpr int bQFull = 0, bQEmpty = 1;
   static constexpr int bKFull = 2, bKEmpty = bKFull + kKStages;
   static constexpr int bVFull = bKEmpty + kKStages, bVEmpty = bVFull + kVStages;
-  static constexpr int bSFull = bVEmpty + kVStages, bPFull = bSFull + kNQ, bODone = bPFull + kNQ;
+  static constexpr int bSFull = bVEmpty + kVStages, bPFull = bSFull + kNQ, bPFullB = bPFull + kNQ, bODone = bPFullB + kNQ;
   static constexpr int bItemFull = bODone + kNQ, bItemEmpty = bItemFull + 2;
   static constexpr int kNumBars = bItemEmpty + 2;
   static constexpr int kInfoOff = kBarOff + ((kNumBars * 8 + 15) / 16) * 16;
@@ -166,11 +166,11 @@ __device__ __forceinline__ uint64_t v_desc(uint32_t tile_addr, int k) {
 }
 
 // compile-time unrolled issue loops (the TMEM offsets must be immediates)
-template <int HD, int Q, int ACC, int K = 0>
+template <int HD, int Q, int ACC, int K, int KEND>
 __device__ __forceinline__ void issue_pv(uint32_t tz, uint32_t vt, uint32_t idesc) {
-  if constexpr (K < kBN / 16) {
+  if constexpr (K < KEND) {
     umma_ts_off<256 + Q * 128, Q * 128 + K * 8>(tz, v_desc<HD>(vt, K), idesc, (ACC) | (K > 0));
-    issue_pv<HD, Q, ACC, K + 1>(tz, vt, idesc);
+    issue_pv<HD, Q, ACC, K + 1, KEND>(tz, vt, idesc);
   }
 }
 template <int HD, int Q, int K = 0>
@@ -205,7 +205,8 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     for (int i = 0; i < S::kVStages; ++i) { mbar_init(bar(S::bVFull + i), kProducerThreads); mbar_init(bar(S::bVEmpty + i), 1); }
     for (int q = 0; q < kNQ; ++q) {
       mbar_init(bar(S::bSFull + q), 1);
-      mbar_init(bar(S::bPFull + q), 128);
+      mbar_init(bar(S::bPFull + q), 128);    // P columns of keys 0..63 written
+      mbar_init(bar(S::bPFullB + q), 128);   // keys 64..127
       mbar_init(bar(S::bODone + q), 1);
     }
     for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 5 + 128 * kNQ); }
@@ -417,18 +418,22 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       // order PV0 QK0 PV1 QK1: the softmax of one tile overlaps the MMAs of the other).  `pending`, `act` and
       // `fresh` come from shared memory, which ptxas cannot prove warp-uniform: they only steer branches, while every
       // MMA operand is built from uniform counters (kst, vst, j) and constants.
-#define SIFT_ISSUE_PV(q, ACC)                                                                                    \
+#define SIFT_ISSUE_PV(q, ACC, K0, K1, LAST)                                                                      \
   if (elect_one()) {                                                                                             \
-    issue_pv<HD, q, ACC>(tz, vt, idesc_pv);                                                                      \
-    umma_commit(bar(S::bODone + q));                                                                             \
+    issue_pv<HD, q, ACC, K0, K1>(tz, vt, idesc_pv);                                                              \
+    if (LAST) umma_commit(bar(S::bODone + q));                                                                   \
   }                                                                                                              \
   __syncwarp();
+  // P of keys 0..63 arrives first: the first half of P V runs while the softmax still works on keys 64..127
 #define SIFT_PV_STEP(q)                                                                                          \
   if (pending & (1 << q)) {                                                                                      \
     mbar_wait(bar(S::bPFull + q), pph[q], 202);                                                                  \
+    tc_fence_after();                                                                                            \
+    if (fresh & (1 << q)) { SIFT_ISSUE_PV(q, 0, 0, kBN / 32, 0) } else { SIFT_ISSUE_PV(q, 1, 0, kBN / 32, 0) }   \
+    mbar_wait(bar(S::bPFullB + q), pph[q], 205);                                                                 \
     pph[q] ^= 1;                                                                                                 \
     tc_fence_after();                                                                                            \
-    if (fresh & (1 << q)) { SIFT_ISSUE_PV(q, 0) } else { SIFT_ISSUE_PV(q, 1) }                                   \
+    SIFT_ISSUE_PV(q, 1, kBN / 32, kBN / 16, 1)                                                                   \
     fresh &= ~(1 << q);                                                                                          \
   }
 #define SIFT_QK_STEP(q)                                                                                          \
@@ -525,7 +530,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         sph ^= 1;
         tc_fence_after();
 #if defined(SIFT_ABL) && SIFT_ABL == 2
-        tc_fence_before(); mbar_arrive(bar(S::bPFull + q)); ++pv_cnt; l = 1.f; m = 0.f; continue;
+        tc_fence_before(); mbar_arrive(bar(S::bPFull + q)); mbar_arrive(bar(S::bPFullB + q)); ++pv_cnt; l = 1.f; m = 0.f; continue;
 #endif
         float s[kBN];
         {
@@ -601,13 +606,18 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
               ::"r"(s_addr + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
                 "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
                 "r"(pk[15]) : "memory");
+          if (c == kBN / 64 - 1) {               // keys 0..63 done: let the first half of P V start
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive(bar(S::bPFull + q));
+          }
         }
         const float2 sum2 = add2(sum_a, sum_b);
         const float sum0 = sum2.x, sum1 = sum2.y;
         l += sum0 + sum1;
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(bar(S::bPFull + q));
+        mbar_arrive(bar(S::bPFullB + q));
         ++pv_cnt;
       }
       // ---- epilogue: O / l -> bf16, LSE
