@@ -29,9 +29,14 @@ namespace sift {
 using namespace ptx;
 
 constexpr int kNQ = SIFT_Q_TILES_PER_ITEM;  // query tiles per work item
-static_assert(kNQ == 2, "the softmax warpgroups split the columns of one tile and alternate between two tiles");
+static_assert(kNQ == 2, "an M-block is two query tiles: two softmax warpgroups, two S and two O accumulators in TMEM");
 constexpr int kBM = 128;                    // rows of one query tile = TMEM lanes
 constexpr int kBN = 128;                    // keys per step
+#ifndef SIFT_PV_PARTS
+#define SIFT_PV_PARTS 4
+#endif
+constexpr int kPvParts = SIFT_PV_PARTS;     // P V is issued in this many key ranges, each as soon as its P is written
+static_assert(kPvParts == 1 || kPvParts == 2 || kPvParts == 4, "P V parts");
 constexpr int kNumThreads = 256 + 128 * kNQ;        // warps 0-3 control/K, softmax warpgroups, 2 V-producer warps, 2 idle
                                                    // (4 warps per SM sub-partition: registers are pooled per sub-partition)
 constexpr int kFirstVWarp = 4 + 4 * kNQ;
@@ -90,7 +95,7 @@ struct Smem {
   static constexpr int bQFull = 0, bQEmpty = 1;
   static constexpr int bKFull = 2, bKEmpty = bKFull + kKStages;
   static constexpr int bVFull = bKEmpty + kKStages, bVEmpty = bVFull + kVStages;
-  static constexpr int bSFull = bVEmpty + kVStages, bPFull = bSFull + kNQ, bPFullB = bPFull + kNQ, bODone = bPFullB + kNQ;
+  static constexpr int bSFull = bVEmpty + kVStages, bPFull = bSFull + kNQ, bODone = bPFull + kNQ * kPvParts;   // bPFull + part * kNQ + q
   static constexpr int bItemFull = bODone + kNQ, bItemEmpty = bItemFull + 2;
   static constexpr int kNumBars = bItemEmpty + 2;
   static constexpr int kInfoOff = kBarOff + ((kNumBars * 8 + 15) / 16) * 16;
@@ -205,8 +210,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     for (int i = 0; i < S::kVStages; ++i) { mbar_init(bar(S::bVFull + i), kProducerThreads); mbar_init(bar(S::bVEmpty + i), 1); }
     for (int q = 0; q < kNQ; ++q) {
       mbar_init(bar(S::bSFull + q), 1);
-      mbar_init(bar(S::bPFull + q), 128);    // P columns of keys 0..63 written
-      mbar_init(bar(S::bPFullB + q), 128);   // keys 64..127
+      for (int part = 0; part < kPvParts; ++part) mbar_init(bar(S::bPFull + part * kNQ + q), 128);   // P of one key range written
       mbar_init(bar(S::bODone + q), 1);
     }
     for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 5 + 128 * kNQ); }
@@ -424,16 +428,21 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     if (LAST) umma_commit(bar(S::bODone + q));                                                                   \
   }                                                                                                              \
   __syncwarp();
-  // P of keys 0..63 arrives first: the first half of P V runs while the softmax still works on keys 64..127
+  // P arrives in kPvParts key ranges: the early parts of P V run while the softmax still works on the later keys
+#define SIFT_PV_PART(q, PART)                                                                                    \
+  if constexpr (PART < kPvParts) {                                                                               \
+    mbar_wait(bar(S::bPFull + PART * kNQ + q), pph[q], 202);                                                     \
+    tc_fence_after();                                                                                            \
+    if (PART == 0 && (fresh & (1 << q))) {                                                                       \
+      SIFT_ISSUE_PV(q, 0, PART * (kBN / 16 / kPvParts), (PART + 1) * (kBN / 16 / kPvParts), PART == kPvParts - 1) \
+    } else {                                                                                                     \
+      SIFT_ISSUE_PV(q, 1, PART * (kBN / 16 / kPvParts), (PART + 1) * (kBN / 16 / kPvParts), PART == kPvParts - 1) \
+    }                                                                                                            \
+  }
 #define SIFT_PV_STEP(q)                                                                                          \
   if (pending & (1 << q)) {                                                                                      \
-    mbar_wait(bar(S::bPFull + q), pph[q], 202);                                                                  \
-    tc_fence_after();                                                                                            \
-    if (fresh & (1 << q)) { SIFT_ISSUE_PV(q, 0, 0, kBN / 32, 0) } else { SIFT_ISSUE_PV(q, 1, 0, kBN / 32, 0) }   \
-    mbar_wait(bar(S::bPFullB + q), pph[q], 205);                                                                 \
+    SIFT_PV_PART(q, 0) SIFT_PV_PART(q, 1) SIFT_PV_PART(q, 2) SIFT_PV_PART(q, 3)                                  \
     pph[q] ^= 1;                                                                                                 \
-    tc_fence_after();                                                                                            \
-    SIFT_ISSUE_PV(q, 1, kBN / 32, kBN / 16, 1)                                                                   \
     fresh &= ~(1 << q);                                                                                          \
   }
 #define SIFT_QK_STEP(q)                                                                                          \
@@ -530,7 +539,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         sph ^= 1;
         tc_fence_after();
 #if defined(SIFT_ABL) && SIFT_ABL == 2
-        tc_fence_before(); mbar_arrive(bar(S::bPFull + q)); mbar_arrive(bar(S::bPFullB + q)); ++pv_cnt; l = 1.f; m = 0.f; continue;
+        tc_fence_before(); for (int part = 0; part < kPvParts; ++part) mbar_arrive(bar(S::bPFull + part * kNQ + q)); ++pv_cnt; l = 1.f; m = 0.f; continue;
 #endif
         float s[kBN];
         {
@@ -606,10 +615,10 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
               ::"r"(s_addr + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
                 "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
                 "r"(pk[15]) : "memory");
-          if (c == kBN / 64 - 1) {               // keys 0..63 done: let the first half of P V start
+          if ((c + 1) % (4 / kPvParts) == 0 && c != kBN / 32 - 1) {   // a key range is done: let its part of P V start
             tmem_wait_st();
             tc_fence_before();
-            mbar_arrive(bar(S::bPFull + q));
+            mbar_arrive(bar(S::bPFull + ((c + 1) / (4 / kPvParts) - 1) * kNQ + q));
           }
         }
         const float2 sum2 = add2(sum_a, sum_b);
@@ -617,7 +626,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         l += sum0 + sum1;
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(bar(S::bPFullB + q));
+        mbar_arrive(bar(S::bPFull + (kPvParts - 1) * kNQ + q));
         ++pv_cnt;
       }
       // ---- epilogue: O / l -> bf16, LSE
