@@ -95,6 +95,8 @@ int sift_decode_metadata(const sift_shape* shape,
  * row strides in elements (head stride = head_dim); bases and row strides 16-byte aligned.
  * O [N][n_q_heads][head_dim] bf16 dev (out); lse [n_q_heads][N] fp32 dev (out, may be NULL): natural-log
  * log-sum-exp of the scaled logits.  A row with no allowed key gets O = 0, lse = -inf.
+ * Environment (read at every call): SIFT_GATHER_MODE=1 gathers the row-granular cross keys with cp.async instead of
+ * TMA tile::gather4 (same results; kept for comparison).
  * softmax_scale <= 0 selects 1/sqrt(head_dim).  fp32 accumulation; P is rounded to bf16 before P*V.
  * Calls that use the same (metadata, layer) must be stream-ordered (they share a work counter). */
 int sift_prefill_attention(const sift_shape* shape, int32_t layer,

@@ -40,9 +40,12 @@ static_assert(kPvParts == 1 || kPvParts == 2 || kPvParts == 4, "P V parts");
 constexpr int kNumThreads = 256 + 128 * kNQ;        // warps 0-3 control/K, softmax warpgroups, 2 V-producer warps, 2 idle
                                                    // (4 warps per SM sub-partition: registers are pooled per sub-partition)
 constexpr int kFirstVWarp = 4 + 4 * kNQ;
-constexpr int kProducerThreads = 64;              // per operand
+constexpr int kProducerThreads = 96;              // per operand: K = warps 2, 3, 14; V = warps 12, 13, 15
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 with a stale max
 constexpr uint32_t kTmemCols = 512;
+#ifndef SIFT_SM_V2
+#define SIFT_SM_V2 0
+#endif
 #ifndef SIFT_EXP_EMU_MASK
 #define SIFT_EXP_EMU_MASK 0x0
 #endif
@@ -73,7 +76,6 @@ struct AttnParams {
   int32_t gather_mode;      // 0: TMA tile::gather4 (default), 1: swizzled cp.async row gather
   const char *k_ptr, *v_ptr;
   int64_t k_row_bytes, v_row_bytes;
-  int32_t debug_no_gather;  // timing experiments only (wrong results): cross groups loaded as tiled boxes
   int32_t n_tokens, n_q_heads, n_kv_heads, tile;
   __nv_bfloat16* o;
   int64_t o_row_stride;
@@ -213,7 +215,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       for (int part = 0; part < kPvParts; ++part) mbar_init(bar(S::bPFull + part * kNQ + q), 128);   // P of one key range written
       mbar_init(bar(S::bODone + q), 1);
     }
-    for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 5 + 128 * kNQ); }
+    for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 7 + 128 * kNQ); }
     fence_barrier_init();
     prefetch_tensormap(&tm_q); prefetch_tensormap(&tm_k); prefetch_tensormap(&tm_v);
     prefetch_tensormap(&tm_kg); prefetch_tensormap(&tm_vg);
@@ -270,7 +272,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       }
       __syncwarp();
     }
-  } else if (warp == 2 || warp == 3 || warp == kFirstVWarp || warp == kFirstVWarp + 1) {
+  } else if (warp == 2 || warp == 3 || warp >= kFirstVWarp) {
     // ======================================= K (warps 2,3) / V (last two warps) producers =======================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
     // 64 threads per operand.  Tiled steps (local tiles, dense rows): one thread issues one TMA box per 64-column half.
@@ -280,8 +282,9 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     // gather_mode 1 (SIFT_GATHER_MODE=1) = every thread copies 16-byte pieces of the listed rows with cp.async,
     // applying the 128-byte swizzle by hand (chunk ^= row & 7) so that the landed image is what a tiled box would
     // have written; completion is signalled by cp.async.mbarrier.arrive.  Both are parity-tested.
-    const bool is_k = warp < 4;
-    const int ptid = is_k ? (int)threadIdx.x - 64 : (int)threadIdx.x - kFirstVWarp * 32;
+    const bool is_k = warp < 4 || warp == kFirstVWarp + 2;
+    const int pw = (warp == kFirstVWarp + 2 || warp == kFirstVWarp + 3) ? 2 : (is_k ? warp - 2 : warp - kFirstVWarp);   // 0..2
+    const int ptid = pw * 32 + lane;
     const int n_stages = is_k ? S::kKStages : S::kVStages;
     const int b_full = is_k ? S::bKFull : S::bVFull, b_empty = is_k ? S::bKEmpty : S::bVEmpty;
     const uint32_t ring = sbase + (is_k ? S::kKOff : S::kVOff);
@@ -307,7 +310,10 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       auto emit = [&](bool gather, int src, int act, bool last) {
         // src: gather -> index of the first cross entry of the group; tiled -> first key row
         const uint32_t full = bar(b_full + st), dst = ring + st * S::kTileBytes;
-        if (gather && p.gather_mode == 1) {
+        if (gather && p.gather_mode == 1 && pw == 2) {
+          mbar_wait(bar(b_empty + st), ph ^ 1, 401);
+          mbar_arrive(full);                     // the third warp only helps with TMA gathers
+        } else if (gather && p.gather_mode == 1) {
           const int32_t* ip = p.cross_idx + (int64_t)it.h * p.cross_cap + src + rr;
           int rows[PCH];
 #pragma unroll
@@ -328,8 +334,11 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           }
           cp_async_mbar_arrive_noinc(full);
         } else {
+          // gather4 slots: 2 halves x 32 groups of 4 rows = 64 per tile, spread 22 / 22 / 20 over the three warps
+          const int g = pw * 22 + lane;
+          const bool g_on = gather && lane < 22 && g < 32 * S::kHalves;
           int4 r = make_int4(0, 0, 0, 0);
-          if (gather) r = *reinterpret_cast<const int4*>(p.cross_idx + (int64_t)it.h * p.cross_cap + src + lane * 4);
+          if (g_on) r = *reinterpret_cast<const int4*>(p.cross_idx + (int64_t)it.h * p.cross_cap + src + (g & 31) * 4);
           mbar_wait(bar(b_empty + st), ph ^ 1, 401);
           if (ptid == 0) {
             if (is_k) info[4 + st] = act | (last ? 4 : 0);
@@ -338,9 +347,8 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             mbar_arrive(full);
           }
           if (gather) {
-            const int hf = ptid >> 5;      // the first warp gathers columns 0..63, the second 64..127
-            if (hf < S::kHalves)
-              tma_gather4(dst + hf * (kBN * 128) + lane * 512, tm_gath, full, it.kvh * HD + hf * 64, r.x, r.y, r.z, r.w);
+            if (g_on)
+              tma_gather4(dst + (g >> 5) * (kBN * 128) + (g & 31) * 512, tm_gath, full, it.kvh * HD + (g >> 5) * 64, r.x, r.y, r.z, r.w);
           } else if (ptid == 0) {
 #pragma unroll
             for (int hf = 0; hf < S::kHalves; ++hf)
@@ -364,7 +372,11 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
         for (int q = 0; q < kNQ; ++q) { present |= (it.rows[q] > 0) << q; nloc += it.lcnt[q]; }
         const int ngroups = (it.cp + kBN - 1) / kBN;
-        for (int g = 0; g < ngroups; ++g) emit(!p.debug_no_gather, g * kBN, present, g == ngroups - 1 && nloc == 0);
+#if defined(SIFT_ABL) && SIFT_ABL == 3   // timing ablation only (wrong results): cross groups loaded as tiled boxes
+        for (int g = 0; g < ngroups; ++g) emit(false, g * kBN, present, g == ngroups - 1 && nloc == 0);
+#else
+        for (int g = 0; g < ngroups; ++g) emit(true, g * kBN, present, g == ngroups - 1 && nloc == 0);
+#endif
         const int32_t* lidx = p.local_idx + (int64_t)it.h * p.local_cap;
         int pos[kNQ];
 #pragma unroll
@@ -559,6 +571,17 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
           for (int c = 0; c < kBN; ++c) s[c] = (c < cur_lim) ? s[c] : -INFINITY;
         }
+#if SIFT_SM_V2 & 1
+        float mx8[8];                                              // eight independent chains of 3-input max
+#pragma unroll
+        for (int j = 0; j < 8; ++j) mx8[j] = fmaxf(s[2 * j], s[2 * j + 1]);
+#pragma unroll
+        for (int c = 16; c < kBN; c += 16) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) mx8[j] = fmaxf(mx8[j], fmaxf(s[c + 2 * j], s[c + 2 * j + 1]));
+        }
+        const float mx = fmaxf(fmaxf(fmaxf(mx8[0], mx8[1]), fmaxf(mx8[2], mx8[3])), fmaxf(fmaxf(mx8[4], mx8[5]), fmaxf(mx8[6], mx8[7])));
+#else
         float mx4[4] = {s[0], s[1], s[2], s[3]};                  // four independent chains
 #pragma unroll
         for (int c = 4; c < kBN; c += 4) {
@@ -566,6 +589,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           mx4[2] = fmaxf(mx4[2], s[c + 2]); mx4[3] = fmaxf(mx4[3], s[c + 3]);
         }
         const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
+#endif
         const float m_new = fmaxf(m, mx);
         const bool need = (m_new - m) * sl > kRescaleThreshold;   // (-inf) - (-inf) = NaN -> false
         if (__any_sync(0xffffffffu, need)) {
@@ -593,10 +617,21 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
         for (int c = 0; c < kBN / 32; ++c) {
           uint32_t pk[16];
+          float2 xq[2];
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
+#if SIFT_SM_V2 & 2
+            // x of pair i+2 is issued (volatile order) before the two ex2 of pair i: the FMA-pipe work rides in the
+            // issue slots the 8-clk MUFU instructions leave free
+            if (i == 0) { xq[0] = fma2v(make_float2(s[c * 32], s[c * 32 + 1]), sl2, nm2); xq[1] = fma2v(make_float2(s[c * 32 + 2], s[c * 32 + 3]), sl2, nm2); }
+            const float2 x = xq[i & 1];
+            if (i + 2 < 16) xq[i & 1] = fma2v(make_float2(s[c * 32 + 2 * i + 4], s[c * 32 + 2 * i + 5]), sl2, nm2);
+            float2 pr;
+            if (true) { pr = make_float2(ex2v(x.x), ex2v(x.y)); } else
+#else
             const float2 x = fma2(make_float2(s[c * 32 + 2 * i], s[c * 32 + 2 * i + 1]), sl2, nm2);
             float2 pr;
+#endif
             if ((kExpEmuMask >> (i & 3)) & 1) {
               pr = ex2_poly2(x);                 // this pair on the FMA pipe: the MUFU is the co-bottleneck (DESIGN 5.2)
             } else {
@@ -789,7 +824,6 @@ extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, co
   p.n_items = lay.n_items; p.n_docs = D; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap;
   p.local_cap = lay.local_cap; p.n_mblocks = lay.n_mblocks;
   p.dense = 0;
-  { const char* e = getenv("SIFT_DEBUG_NO_GATHER"); p.debug_no_gather = (e && e[0] == '1'); }
   p.n_tokens = shape->doc_offsets[D] + shape->query_len;
   p.n_q_heads = Hq; p.n_kv_heads = shape->n_kv_heads; p.tile = shape->tile;
   p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
