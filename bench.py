@@ -131,7 +131,7 @@ class GpuCase:
         self.decode()
         torch.cuda.synchronize()
         views = {k_: t.cpu().numpy() for k_, t in api.metadata_views(self.shape, self.md).items()}
-        self.pairs = int(metrics.marked_pairs_per_head(views, layer, w.shape.n_docs).sum())
+        self.pairs = int(metrics.marked_pairs_per_head(views, layer, w.shape.n_docs, w.shape.cross_gran).sum())
         self.flops = metrics.attention_flops(self.pairs, w.shape.head_dim)
         self.dense_flops = metrics.attention_flops(metrics.dense_causal_pairs(w.shape.n_tokens) * w.shape.n_q_heads,
                                                    w.shape.head_dim)

@@ -40,7 +40,7 @@ extern "C" {
 typedef enum {
   SIFT_OK = 0,
   SIFT_ERR_INVALID_ARG = -1, /* NULL pointer, non-increasing offsets, misaligned tensor, ... */
-  SIFT_ERR_UNSUPPORTED = -2, /* head_dim not in {64,128}, tile not in {64,128}, cross_gran != 1, n_docs > SIFT_MAX_DOCS */
+  SIFT_ERR_UNSUPPORTED = -2, /* head_dim not in {64,128}, tile not in {64,128}, cross_gran not in {1,tile}, n_docs > SIFT_MAX_DOCS */
   SIFT_ERR_WORKSPACE = -3,   /* metadata buffer too small */
   SIFT_ERR_CUDA = -4         /* launch / driver error */
 } sift_status;
@@ -50,7 +50,7 @@ typedef struct {
   int32_t n_layers, n_q_heads, n_kv_heads, head_dim;
   int32_t n_docs, query_len;
   int32_t tile;       /* T: 64 or 128 (M-block = N-block = T) */
-  int32_t cross_gran; /* G: 1 = one CA bit per key token (BASELINE.json configs) */
+  int32_t cross_gran; /* G: 1 = one CA bit per key token (BASELINE.json configs); tile = one bit per page */
   const int32_t* doc_offsets; /* HOST, n_docs + 1 entries */
 } sift_shape;
 
@@ -59,14 +59,15 @@ typedef struct {
  *   tile_base [n_docs+2]           first global tile id of each segment; tile_base[n_docs+1] = NT
  *   tile_seg/tile_row0/tile_rows [NT]
  *   cross_ptr [L][Hq][n_docs+1]    cross_ptr[d] = number of marked keys in documents 0..d-1
- *   cross_idx [L][Hq][cross_cap]   ascending global key rows; rows of document d attend entries [0, cross_ptr[d])
+ *   cross_idx [L][Hq][cross_cap]   ascending global key rows (G = 1) or global tile ids (G = tile); rows of
+ *                                  document d attend entries [0, cross_ptr[d])
  *   local_cnt [L][Hq][NT], local_ptr [L][Hq][NT+1], local_idx [L][Hq][local_cap]
  *                                  per M-block: ascending global tile ids of marked LA tiles; query M-block t: 0..t
  * Private arrays (scheduler): sched [L][n_items], counters [L][2]. */
 typedef struct {
   uint32_t struct_size;
   int32_t n_tiles;   /* NT */
-  int32_t cross_cap; /* per (layer, head) stride of cross_idx, multiple of 128 */
+  int32_t cross_cap; /* per (layer, head) stride of cross_idx: sum_d ceil(len_d / G) rounded up to 128 */
   int32_t local_cap; /* per (layer, head) stride of local_idx */
   int32_t n_mblocks; /* scheduler M-blocks per head */
   int32_t n_items;   /* work items per layer = n_q_heads * n_mblocks */

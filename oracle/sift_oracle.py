@@ -272,8 +272,11 @@ def tile_tables(doc_offsets: Sequence[int], query_len: int, tile: int) -> Dict[s
 
 
 def cross_capacity(doc_offsets: Sequence[int], gran: int) -> int:
-    """ceil(off[D]/G) rounded up to a multiple of 128 (SURVEY.md 8(c) MD-v1)."""
-    n = -(-int(doc_offsets[-1]) // gran)
+    """sum over documents of ceil(L_d / G), rounded up to a multiple of 128 (MD-v1, reading R5: SURVEY.md
+    8(c) wrote ceil(off[D]/G), which is the same number for G = 1 but too small for G = tile with ragged documents,
+    where every document contributes ceil(L_d / tile) pages)."""
+    off = [int(x) for x in doc_offsets]
+    n = sum(-(-(off[d + 1] - off[d]) // gran) for d in range(len(off) - 1))
     return -(-n // 128) * 128
 
 

@@ -77,6 +77,7 @@ struct AttnParams {
   const char *k_ptr, *v_ptr;
   int64_t k_row_bytes, v_row_bytes;
   int32_t n_tokens, n_q_heads, n_kv_heads, tile;
+  int32_t paged;            // cross_gran == tile: cross entries are global tile ids, one tiled step each
   __nv_bfloat16* o;
   int64_t o_row_stride;
   float* lse;  // [Hq][N] or null
@@ -371,7 +372,11 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         int present = 0, nloc = 0;
 #pragma unroll
         for (int q = 0; q < kNQ; ++q) { present |= (it.rows[q] > 0) << q; nloc += it.lcnt[q]; }
-        const int ngroups = (it.cp + kBN - 1) / kBN;
+        const int ngroups = p.paged ? 0 : (it.cp + kBN - 1) / kBN;
+        if (p.paged) {                     // page-granular cross keys: the listed pages as tiled boxes
+          const int32_t* cidx = p.cross_idx + (int64_t)it.h * p.cross_cap;
+          for (int e = 0; e < it.cp; ++e) emit(false, p.tile_row0[cidx[e]], present, e == it.cp - 1 && nloc == 0);
+        }
 #if defined(SIFT_ABL) && SIFT_ABL == 3   // timing ablation only (wrong results): cross groups loaded as tiled boxes
         for (int g = 0; g < ngroups; ++g) emit(false, g * kBN, present, g == ngroups - 1 && nloc == 0);
 #else
@@ -528,13 +533,14 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       mbar_arrive(bar(S::bItemEmpty + slot));
       if (code < 0) break;
       int row0, rows, h, ngroups, nsteps, diag_step, lim;
+      bool paged_item;
       {
         const Item it = load_item(p, code);
         row0 = q ? it.row0[1] : it.row0[0]; rows = q ? it.rows[1] : it.rows[0]; h = it.h;
         const int lcnt = q ? it.lcnt[1] : it.lcnt[0], lptr = q ? it.lptr[1] : it.lptr[0];
         const int tile_id = q ? it.tile_id[1] : it.tile_id[0];
         if (rows <= 0) continue;
-        ngroups = it.is_dense ? 0 : (it.cp + kBN - 1) / kBN;
+        ngroups = it.is_dense ? 0 : (p.paged ? it.cp : (it.cp + kBN - 1) / kBN);
         nsteps = it.is_dense ? dense_steps(row0, rows) : ngroups + lcnt;
         diag_step = -1;                                   // the step (if any) that is the causally masked diagonal tile
         if (!it.is_dense && lcnt > 0 && p.local_idx[(int64_t)h * p.local_cap + lptr + lcnt - 1] == tile_id)
@@ -543,10 +549,12 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         // phase (ragged last group) and in DENSE items (causal frontier)
         lim = it.is_dense ? row0 + r + 1 : it.cp;
         if (it.is_dense) ngroups = nsteps;                // "frontier" steps: all of them
+        paged_item = p.paged && !it.is_dense;
       }
       float m = -INFINITY, l = 0.f;
       for (int e = 0; e < nsteps; ++e, lim -= kBN) {
-        const int cur_lim = (e < ngroups) ? lim : (e == diag_step ? min(tile_lim, r + 1) : tile_lim);
+        int cur_lim = (e < ngroups) ? lim : (e == diag_step ? min(tile_lim, r + 1) : tile_lim);
+        if (paged_item && e < ngroups) cur_lim = p.tile_rows[p.cross_idx[(int64_t)h * p.cross_cap + e]];   // a page may be ragged
         mbar_wait(bar(S::bSFull + q), sph, 301);
         sph ^= 1;
         tc_fence_after();
@@ -826,6 +834,7 @@ extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, co
   p.dense = 0;
   p.n_tokens = shape->doc_offsets[D] + shape->query_len;
   p.n_q_heads = Hq; p.n_kv_heads = shape->n_kv_heads; p.tile = shape->tile;
+  p.paged = (shape->cross_gran != 1);
   p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
   const float sc = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf((float)HD);
   p.scale_log2 = sc * 1.4426950408889634f;

@@ -26,7 +26,7 @@ struct DecodeParams {
   int32_t *tile_base, *tile_seg, *tile_row0, *tile_rows;
   int32_t *cross_ptr, *cross_idx, *local_cnt, *local_ptr, *local_idx;
   int32_t *mblock_tile0, *sched, *counters;
-  int32_t n_q_heads, n_tiles, cross_cap, local_cap, n_mblocks, n_items;
+  int32_t n_q_heads, n_tiles, cross_cap, local_cap, n_mblocks, n_items, gran;
 };
 
 // exclusive scan over the block; returns the exclusive prefix of v and (via total) the block sum
@@ -239,7 +239,8 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
         uint32_t m = (hi >= 32) ? 0xffffffffu : ((1u << hi) - 1u);
         m &= ~((lo >= 32) ? 0xffffffffu : ((1u << lo) - 1u));
         bits[k] = x & m;
-        key0[k] = dt.off[d] + wi * 32 - lead;   // G == 1: global key row of stream bit 0 of this word
+        // global coordinate of stream bit 0 of this word: key row (G == 1) or tile id (G == tile; a page is a tile)
+        key0[k] = (G == 1 ? dt.off[d] : s_tile_base[d]) + wi * 32 - lead;
         if (v + 1 == s_wstart[d + 1]) dd[k] = d;   // last word of document d
       }
     }
@@ -351,7 +352,8 @@ sift_schedule_kernel(const DecodeParams p, int n_docs, int n_layers_unused) {
     const int seg = p.tile_seg[t0];
     int c = 0;
     for (int t = t0; t < t1; ++t) {
-      if (seg < D) c += (p.cross_ptr[lh * (D + 1) + seg] + 127) / 128 + p.local_cnt[lh * NT + t];
+      // steps of a document tile: groups of 128 gathered rows (G == 1) or one page per step (G == tile), plus local tiles
+      if (seg < D) c += (p.gran == 1 ? (p.cross_ptr[lh * (D + 1) + seg] + 127) / 128 : p.cross_ptr[lh * (D + 1) + seg]) + p.local_cnt[lh * NT + t];
       else c += (p.tile_row0[t] + p.tile_rows[t] + 127) / 128;
     }
     return min(c, kCostBuckets - 1);
@@ -409,7 +411,7 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   p.local_cnt = at(lay.local_cnt); p.local_ptr = at(lay.local_ptr); p.local_idx = at(lay.local_idx);
   p.mblock_tile0 = at(lay.mblock_tile0); p.sched = at(lay.sched); p.counters = at(lay.counters);
   p.n_q_heads = s->n_q_heads; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap; p.local_cap = lay.local_cap;
-  p.n_mblocks = lay.n_mblocks; p.n_items = lay.n_items;
+  p.n_mblocks = lay.n_mblocks; p.n_items = lay.n_items; p.gran = s->cross_gran;
   cudaGetLastError();
   sift_decode_lists_kernel<<<dim3(s->n_q_heads, s->n_layers), kDecodeThreads, 0, st>>>(dt, p);
   sift_schedule_kernel<<<s->n_layers, kSchedThreads, 0, st>>>(p, s->n_docs, s->n_layers);

@@ -32,8 +32,8 @@ int validate_shape(const sift_shape* s) {
   if (s->head_dim != 64 && s->head_dim != 128)
     return set_error(SIFT_ERR_UNSUPPORTED, "head_dim %d not in {64,128}", s->head_dim);
   if (s->tile != 64 && s->tile != 128) return set_error(SIFT_ERR_UNSUPPORTED, "tile %d not in {64,128}", s->tile);
-  if (s->cross_gran != 1)
-    return set_error(SIFT_ERR_UNSUPPORTED, "cross_gran %d: only 1 (per key token) is built", s->cross_gran);
+  if (s->cross_gran != 1 && s->cross_gran != s->tile)
+    return set_error(SIFT_ERR_UNSUPPORTED, "cross_gran %d: 1 (per key token) or tile (per page, PAPER.md:L209)", s->cross_gran);
   if (s->n_docs > SIFT_MAX_DOCS) return set_error(SIFT_ERR_UNSUPPORTED, "n_docs %d > %d", s->n_docs, SIFT_MAX_DOCS);
   if (s->doc_offsets[0] != 0) return set_error(SIFT_ERR_INVALID_ARG, "doc_offsets[0] != 0");
   for (int d = 0; d < s->n_docs; ++d)
@@ -50,9 +50,10 @@ int compute_layout(const sift_shape* s, sift_md_layout* out) {
   int rc = validate_shape(s);
   if (rc) return rc;
   const int T = s->tile, D = s->n_docs, NQ = SIFT_Q_TILES_PER_ITEM;
-  int64_t nt = 0, lcap = 0, nmb = 0;
+  int64_t nt = 0, lcap = 0, nmb = 0, ncross = 0;
   for (int d = 0; d < D; ++d) {
     int64_t p = ceil_div_i(s->doc_offsets[d + 1] - s->doc_offsets[d], T);
+    ncross += ceil_div_i(s->doc_offsets[d + 1] - s->doc_offsets[d], s->cross_gran);
     nt += p;
     lcap += p * (p + 1) / 2;
     nmb += (p + NQ - 1) / NQ;
@@ -61,7 +62,7 @@ int compute_layout(const sift_shape* s, sift_md_layout* out) {
   for (int64_t t = nt; t < nt + pq; ++t) lcap += t + 1;
   nt += pq;
   nmb += (pq + NQ - 1) / NQ;
-  int64_t ccap = (int64_t)ceil_div_i(ceil_div_i(s->doc_offsets[D], s->cross_gran), 128) * 128;
+  int64_t ccap = (ncross + 127) / 128 * 128;   // one entry per CA bit at most, rounded up to whole gather groups
   if (lcap >= (1ll << 31) || ccap >= (1ll << 31)) return set_error(SIFT_ERR_UNSUPPORTED, "index capacity >= 2^31");
   if (lcap < 1) lcap = 1;
   const int64_t LH = (int64_t)s->n_layers * s->n_q_heads;

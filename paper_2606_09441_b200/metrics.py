@@ -7,7 +7,7 @@ from typing import Dict
 import numpy as np
 
 
-def marked_pairs_per_head(md: Dict[str, np.ndarray], layer: int, n_docs: int) -> np.ndarray:
+def marked_pairs_per_head(md: Dict[str, np.ndarray], layer: int, n_docs: int, cross_gran: int = 1) -> np.ndarray:
     """True mask entries per q-head of one layer (reading A26: element level; the diagonal tile counts its causal
     half, ragged tiles their real rows).  md: numpy views of the MD-v1 arrays."""
     seg, row0, rows = md["tile_seg"], md["tile_row0"].astype(np.int64), md["tile_rows"].astype(np.int64)
@@ -17,7 +17,12 @@ def marked_pairs_per_head(md: Dict[str, np.ndarray], layer: int, n_docs: int) ->
     is_doc = seg < n_docs
     for h in range(n_heads):
         cp = md["cross_ptr"][layer, h].astype(np.int64)
-        tot = int((rows[is_doc] * cp[seg[is_doc]]).sum())
+        if cross_gran == 1:                          # entries are key rows
+            keys_before = cp
+        else:                                        # entries are pages: a page contributes its real rows
+            ci = md["cross_idx"][layer, h][: cp[-1]].astype(np.int64)
+            keys_before = np.concatenate([[0], np.cumsum(rows[ci])])[cp]
+        tot = int((rows[is_doc] * keys_before[seg[is_doc]]).sum())
         lp = md["local_ptr"][layer, h].astype(np.int64)
         li = md["local_idx"][layer, h]
         owner = np.repeat(np.arange(nt), np.diff(lp))

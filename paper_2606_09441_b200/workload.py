@@ -252,10 +252,11 @@ def config_8b_10k(seed: int = BASE_SEED) -> Workload:
                           recipe="10x1024+128, T=128, p_loc~U(.2,.4), p_cross~U(.1,.3) per head")
 
 
-def config_32k(seed: int = BASE_SEED, n_layers: int = 1) -> Workload:
-    sh = PromptShape(n_layers, 32, 8, 128, (2000,) * 16, 256, tile=128, cross_gran=1)
+def config_32k(seed: int = BASE_SEED, n_layers: int = 1, cross_gran: int = 1) -> Workload:
+    sh = PromptShape(n_layers, 32, 8, 128, (2000,) * 16, 256, tile=128, cross_gran=cross_gran)
     pl, pc = _beta_dens(seed, n_layers, 32)
-    return build_workload("C3-32k" if n_layers == 1 else f"C5-stack{n_layers}", sh, seed, pl, pc,
+    name = ("C3-32k" if n_layers == 1 else f"C5-stack{n_layers}") + ("" if cross_gran == 1 else "-paged")
+    return build_workload(name, sh, seed, pl, pc,
                           recipe="16x2000+256, T=128, p_loc~Beta(2,6), p_cross~Beta(2,8) per (layer, head)")
 
 
@@ -308,6 +309,8 @@ CONFIGS: Dict[str, Callable[[], Workload]] = {
     "32k": config_32k,
     "64k-ragged": config_64k_ragged,
     "full-stack": config_full_stack,
+    # the paper's page-granular CA (one bit per 128-key page) on C3's shape, same densities per bit
+    "32k-paged": lambda seed=BASE_SEED: config_32k(seed, cross_gran=128),
 }
 
 

@@ -26,7 +26,7 @@ def test_exports_match_header():
     assert "sift-b200" in api.sift_version()
 
 
-@pytest.mark.parametrize("cfg", ["tiny", "8b-10k", "32k", "64k-ragged"])
+@pytest.mark.parametrize("cfg", ["tiny", "8b-10k", "32k", "64k-ragged", "32k-paged"])
 def test_layout_matches_oracle_capacities(cfg):
     w = wl.CONFIGS[cfg]()
     sh = w.shape
@@ -45,7 +45,8 @@ def test_bad_arguments_rejected():
     good = dict(n_layers=1, n_q_heads=4, n_kv_heads=2, head_dim=64, doc_offsets=np.array([0, 100, 200]), query_len=10,
                 tile=64)
     api.sift_metadata_size(api.Shape(**good))
-    for bad in (dict(head_dim=96), dict(tile=32), dict(cross_gran=64), dict(n_kv_heads=3),
+    api.sift_metadata_size(api.Shape(**{**good, "cross_gran": 64}))    # page-granular CA: G = tile
+    for bad in (dict(head_dim=96), dict(tile=32), dict(cross_gran=32), dict(n_kv_heads=3),
                 dict(doc_offsets=np.array([0, 100, 100])), dict(doc_offsets=np.array([1, 100])),
                 dict(doc_offsets=np.arange(0, 64 * 600, 64))):
         with pytest.raises(api.SiftError):

@@ -31,6 +31,10 @@ def test_decode_bit_exact_configs(cfg):
     dict(doc_lens=(300, 200), query_len=70, tile=128, p_loc=-1.0, p_cross=-1.0, diag_set=False),
     dict(doc_lens=tuple([37] * 300), query_len=5, tile=64, n_q_heads=1),
     dict(doc_lens=(9000,), query_len=100, tile=64, n_q_heads=1),
+    # page-granular CA (G = tile): entries are global tile ids
+    dict(doc_lens=(63, 64, 65, 1, 129), query_len=1, tile=64, cross_gran=64),
+    dict(doc_lens=(2000, 1500, 700), query_len=100, tile=128, cross_gran=128, n_layers=2, n_q_heads=4, n_kv_heads=2),
+    dict(doc_lens=tuple([37] * 300), query_len=5, tile=64, n_q_heads=1, cross_gran=64, p_cross=0.6),
 ])
 def test_decode_bit_exact_edge_cases(case):
     w = wl.custom("edge", seed=41, **case)
@@ -87,6 +91,25 @@ def test_cross_gather_cp_async_mode(case, monkeypatch):
     w = wl.custom("cross-cpasync", seed=23, **case)
     _, _, o, lse = gu.run_sift(w)
     _report(f"cp.async gather {case}", gu.attention_errors(w, 0, o, lse, range(w.shape.n_q_heads), range(w.shape.n_tokens)))
+
+
+@pytest.mark.parametrize("case", [
+    dict(n_q_heads=4, n_kv_heads=2, head_dim=128, doc_lens=(384, 300, 700, 130), query_len=140, tile=128, cross_gran=128, p_cross=0.5),
+    dict(n_q_heads=2, n_kv_heads=1, head_dim=64, doc_lens=(256, 300, 129, 64), query_len=33, tile=64, cross_gran=64, p_cross=0.4),
+])
+def test_paged_cross_all_rows(case):
+    """page-granular CA (one bit per tile of keys), cross pages loaded as tiled TMA boxes."""
+    w = wl.custom("paged", seed=29, **case)
+    shape, md, o, lse = gu.run_sift(w)
+    gu.assert_metadata_equal(w, shape, md)
+    _report(f"paged {case}", gu.attention_errors(w, 0, o, lse, range(w.shape.n_q_heads), range(w.shape.n_tokens)))
+
+
+def test_paged_32k_sampled_rows():
+    w = wl.CONFIGS["32k-paged"]()
+    _, _, o, lse = gu.run_sift(w)
+    assert torch.isfinite(o.float()).all()
+    _report("32k-paged", gu.attention_errors(w, 0, o, lse, [3, 30], gu.sample_rows(w)))
 
 
 def test_empty_rows_A13():

@@ -39,3 +39,19 @@ def test_determinism_and_reorder_views():
     assert np.array_equal(r.la_vec(0, 1, 0), a.la_vec(0, 1, 3)) and np.array_equal(r.ca_vec(0, 0, 2), a.ca_vec(0, 0, 0))
     qr, kr, vr = r.qkv(0)
     assert qr[0:256].equal(qa[768:1024]) and kr[512:768].equal(ka[0:256]) and qr[1024:].equal(qa[1024:])
+
+
+def test_marked_pairs_metric_matches_oracle_mask_count():
+    """bench.py's pair count (integer arithmetic over MD-v1 arrays) against the oracle's explicit mask, G = 1 and G = tile."""
+    import pytest
+    from oracle import sift_oracle as so
+    from paper_2606_09441_b200 import metrics
+    for gran in (1, 16):
+        w = wl.custom("pairs", doc_lens=(50, 33, 16, 70), query_len=21, tile=16, cross_gran=gran, p_loc=0.4, p_cross=0.35,
+                      n_q_heads=2, seed=5)
+        sh = w.shape
+        md = so.decode_metadata(sh.doc_offsets, sh.query_len, sh.tile, gran, 1, 2, w.la_vec, w.ca_vec)
+        got = metrics.marked_pairs_per_head(md, 0, sh.n_docs, gran)
+        for h in range(2):
+            la, ca = so.head_vectors(w, 0, h)
+            assert int(got[h]) == so.marked_pairs(sh.doc_offsets, sh.query_len, sh.tile, gran, la, ca)
