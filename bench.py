@@ -400,7 +400,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": float(np.mean(secs)) * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{w.name}: {w.recipe}", "n_tokens": w.shape.n_tokens},
+        "config": {"workload": f"BASELINE.json configs[2] 32K context: {w.recipe}" if args.config == "32k" else w.name + ": " + w.recipe,
+                   "n_tokens": w.shape.n_tokens, "heads": f"{w.shape.n_q_heads}/{w.shape.n_kv_heads}", "head_dim": w.shape.head_dim},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": "each step: " + what},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
