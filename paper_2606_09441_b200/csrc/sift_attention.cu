@@ -77,6 +77,7 @@ struct AttnParams {
   const char *k_ptr, *v_ptr;
   int64_t k_row_bytes, v_row_bytes;
   int32_t n_tokens, n_q_heads, n_kv_heads, tile;
+  int32_t kv_per_group;     // dense comparator: kv heads scheduled together (sched_kv_heads_per_group)
   int32_t paged;            // cross_gran == tile: cross entries are global tile ids, one tiled step each
   __nv_bfloat16* o;
   int64_t o_row_stride;
@@ -249,7 +250,14 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       if (lane == 0) {
         const int idx = atomicAdd(&p.counters[0], 1);
         if (idx < p.n_items) {
-          code = p.dense ? (((idx % p.n_q_heads) << 20) | (p.n_mblocks - 1 - idx / p.n_q_heads)) : p.sched[idx];
+          if (p.dense) {   // kv-head groups one after the other, longest M-blocks first inside a group
+            const int hpg = (p.n_q_heads / p.n_kv_heads) * p.kv_per_group, per_group = hpg * p.n_mblocks;   // (last group may be short)
+            const int g = idx / per_group, rem = idx - g * per_group;
+            const int hin = min(hpg, p.n_q_heads - g * hpg);   // q-heads in this group
+            code = ((g * hpg + rem % hin) << 20) | (p.n_mblocks - 1 - rem / hin);
+          } else {
+            code = p.sched[idx];
+          }
         } else {
           const int f = atomicAdd(&p.counters[1], 1);
           if (f == (int)gridDim.x - 1) { atomicExch(&p.counters[0], 0); atomicExch(&p.counters[1], 0); }
@@ -858,6 +866,7 @@ extern "C" int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, 
   p.dense = 1;
   p.n_tokens = n_tokens; p.n_q_heads = n_q_heads; p.n_kv_heads = n_kv_heads; p.tile = 128;
   p.n_mblocks = (n_tokens + kBM * kNQ - 1) / (kBM * kNQ);
+  p.kv_per_group = sched_kv_heads_per_group(n_tokens, head_dim, n_kv_heads);
   p.n_items = p.n_mblocks * n_q_heads;
   void* cptr = nullptr;
   if (cudaGetSymbolAddress(&cptr, g_dense_counters) != cudaSuccess) return set_error(SIFT_ERR_CUDA, "no device symbol");

@@ -26,7 +26,8 @@ struct DecodeParams {
   int32_t *tile_base, *tile_seg, *tile_row0, *tile_rows;
   int32_t *cross_ptr, *cross_idx, *local_cnt, *local_ptr, *local_idx;
   int32_t *mblock_tile0, *sched, *counters;
-  int32_t n_q_heads, n_tiles, cross_cap, local_cap, n_mblocks, n_items, gran;
+  int32_t n_q_heads, n_kv_heads, n_tiles, cross_cap, local_cap, n_mblocks, n_items, gran;
+  int32_t kv_per_group;   // kv heads whose work items are scheduled together (sched_kv_heads_per_group)
 };
 
 // exclusive scan over the block; returns the exclusive prefix of v and (via total) the block sum
@@ -334,8 +335,8 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
   if (tid == 0) local_ptr[NT] = running;
 }
 
-// Work items (head, M-block) of one layer sorted by descending cost (counting sort): the persistent
-// attention grid pulls them through an atomic counter, longest first.
+// Work items (head, M-block) of one layer sorted by (kv-head group, descending cost) (counting sort): the persistent
+// attention grid pulls them through an atomic counter.
 __global__ void __launch_bounds__(kSchedThreads)
 sift_schedule_kernel(const DecodeParams p, int n_docs, int n_layers_unused) {
   __shared__ int s_hist[kCostBuckets];
@@ -356,7 +357,12 @@ sift_schedule_kernel(const DecodeParams p, int n_docs, int n_layers_unused) {
       if (seg < D) c += (p.gran == 1 ? (p.cross_ptr[lh * (D + 1) + seg] + 127) / 128 : p.cross_ptr[lh * (D + 1) + seg]) + p.local_cnt[lh * NT + t];
       else c += (p.tile_row0[t] + p.tile_rows[t] + 127) / 128;
     }
-    return min(c, kCostBuckets - 1);
+    // bucket = processing order: groups of kv heads one after the other (the q-heads of a kv head gather from the same
+    // K/V, so the K/V working set of the grid stays L2-sized and K/V are read from HBM about once), longest items
+    // first inside a group
+    const int groups = (p.n_kv_heads + p.kv_per_group - 1) / p.kv_per_group, bpg = kCostBuckets / groups;
+    const int g = h / (p.n_q_heads / p.n_kv_heads) / p.kv_per_group;
+    return g * bpg + (bpg - 1 - min(c, bpg - 1));
   };
   // the cost of an item is a chain of dependent global loads: evaluate it once and keep it in registers for the
   // scatter pass (up to kCached items per thread; larger layers recompute)
@@ -369,11 +375,11 @@ sift_schedule_kernel(const DecodeParams p, int n_docs, int n_layers_unused) {
   }
 #pragma unroll
   for (int k = 0; k < kCached; ++k)
-    if (tid + k * kSchedThreads < p.n_items) atomicAdd(&s_hist[kCostBuckets - 1 - ccost[k]], 1);
+    if (tid + k * kSchedThreads < p.n_items) atomicAdd(&s_hist[ccost[k]], 1);
   for (int e = tid + kCached * kSchedThreads; e < p.n_items; e += kSchedThreads)
-    atomicAdd(&s_hist[kCostBuckets - 1 - cost_of(e)], 1);
+    atomicAdd(&s_hist[cost_of(e)], 1);
   __syncthreads();
-  {  // exclusive scan over buckets (bucket 0 = highest cost)
+  {  // exclusive scan over buckets (bucket 0 = first to be processed)
     constexpr int PER = kCostBuckets / kSchedThreads;
     int loc[PER], sum = 0;
 #pragma unroll
@@ -387,7 +393,7 @@ sift_schedule_kernel(const DecodeParams p, int n_docs, int n_layers_unused) {
   int32_t* sched = p.sched + (int64_t)l * p.n_items;
   auto place = [&](int e, int c) {
     const int h = e / NMB, mb = e - h * NMB;
-    const int pos = atomicAdd(&s_hist[kCostBuckets - 1 - c], 1);
+    const int pos = atomicAdd(&s_hist[c], 1);
     sched[pos] = (h << 20) | mb;
   };
 #pragma unroll
@@ -410,8 +416,9 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   p.cross_ptr = at(lay.cross_ptr); p.cross_idx = at(lay.cross_idx);
   p.local_cnt = at(lay.local_cnt); p.local_ptr = at(lay.local_ptr); p.local_idx = at(lay.local_idx);
   p.mblock_tile0 = at(lay.mblock_tile0); p.sched = at(lay.sched); p.counters = at(lay.counters);
-  p.n_q_heads = s->n_q_heads; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap; p.local_cap = lay.local_cap;
+  p.n_q_heads = s->n_q_heads; p.n_kv_heads = s->n_kv_heads; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap; p.local_cap = lay.local_cap;
   p.n_mblocks = lay.n_mblocks; p.n_items = lay.n_items; p.gran = s->cross_gran;
+  p.kv_per_group = sched_kv_heads_per_group((int64_t)s->doc_offsets[s->n_docs] + s->query_len, s->head_dim, s->n_kv_heads);
   cudaGetLastError();
   sift_decode_lists_kernel<<<dim3(s->n_q_heads, s->n_layers), kDecodeThreads, 0, st>>>(dt, p);
   sift_schedule_kernel<<<s->n_layers, kSchedThreads, 0, st>>>(p, s->n_docs, s->n_layers);
