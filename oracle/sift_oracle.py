@@ -419,3 +419,76 @@ def marked_pairs(doc_offsets: Sequence[int], query_len: int, tile: int, gran: in
 def head_vectors(w, layer: int, head: int) -> Tuple[List[np.ndarray], List[np.ndarray]]:
     n_docs = len(w.shape.doc_lens)
     return ([w.la_vec(layer, head, d) for d in range(n_docs)], [w.ca_vec(layer, head, d) for d in range(n_docs)])
+
+
+# ------------------------------------------------------------------------------------------
+# Part 4: offline metadata generation (sec 4.1, L209 sec 4.2, L223 sec 4.4)
+# ------------------------------------------------------------------------------------------
+# Plain definition, fp64: the standalone dense causal attention of ONE document gives a probability matrix p[q, k]
+# (k <= q).  LA tile (i, j) is marked iff it holds at least one p >= alpha (L201).  CA (reading R6 of DESIGN.md; the
+# paper words it per page at L209 and per key token at L185): a key group g (one key at G = 1, T keys at G = tile) is
+# marked iff hits(g) > gamma * cells(g), hits = causal cells of its key columns with p >= beta, cells = all causal
+# cells of those columns.  Pins (tests/test_oracle_pins.py): q = 0 gives p = 1/(q+1) in closed form; one-hot attention
+# gives the diagonal-only LA vector 0xA4 of the paper's enumeration; alpha <= min p marks every tile.
+
+def pack_bits_msb(bits: Sequence[int]) -> np.ndarray:
+    """MSB-first packing, padded with zeros to the next byte boundary."""
+    out = np.zeros((len(bits) + 7) // 8, dtype=np.uint8)
+    for n, b in enumerate(bits):
+        if b:
+            out[n >> 3] |= 0x80 >> (n & 7)
+    return out
+
+
+def document_probabilities(q_doc: torch.Tensor, k_doc: torch.Tensor, scale: Optional[float] = None) -> np.ndarray:
+    """p[q, k] of the dense causal attention of one document and head; q_doc, k_doc [L, d]; fp64; 0 above the diagonal."""
+    n, d = q_doc.shape
+    if scale is None:
+        scale = 1.0 / math.sqrt(d)
+    s = (q_doc.to(torch.float64) @ k_doc.to(torch.float64).T) * scale
+    causal = torch.tril(torch.ones((n, n), dtype=torch.bool))
+    s = torch.where(causal, s, torch.full_like(s, -math.inf))
+    p = torch.softmax(s, dim=1)
+    return p.numpy()
+
+
+def encode_from_probabilities(p: np.ndarray, tile: int, gran: int, alpha: float, beta: float, gamma: float
+                              ) -> Tuple[np.ndarray, np.ndarray, Dict[str, np.ndarray]]:
+    """LA and CA vectors (packed) of one (document, head) from its probability matrix, plus the unpacked decisions
+    and their margins (used by the GPU parity test to set aside cells that sit on a threshold)."""
+    n = p.shape[0]
+    pt = pages(n, tile)
+    la_bits, la_max = [], []
+    for i in range(pt):
+        for j in range(i + 1):
+            blk = p[i * tile: min(n, (i + 1) * tile), j * tile: min(n, (j + 1) * tile)]
+            if i == j:
+                blk = np.tril(blk)                       # cells above the diagonal are not part of the tile's triangle
+            mx = float(blk.max())
+            la_bits.append(1 if mx >= alpha else 0)
+            la_max.append(mx)
+    n_groups = -(-n // gran)
+    hit = (p >= beta) & np.tril(np.ones((n, n), dtype=bool))
+    col_hits = hit.sum(axis=0).astype(np.int64)          # per key column
+    ca_bits, hits_g, cells_g = [], [], []
+    g32 = float(np.float32(gamma))                       # the library receives gamma as fp32 and decides in fp64
+    for g in range(n_groups):
+        ks = range(g * gran, min(n, (g + 1) * gran))
+        hits = int(sum(int(col_hits[k]) for k in ks))
+        cells = int(sum(n - k for k in ks))
+        ca_bits.append(1 if hits > g32 * cells else 0)
+        hits_g.append(hits)
+        cells_g.append(cells)
+    info = {"la_bits": np.array(la_bits), "la_max": np.array(la_max), "ca_bits": np.array(ca_bits),
+            "hits": np.array(hits_g), "cells": np.array(cells_g), "col_hits": col_hits}
+    return pack_bits_msb(la_bits), pack_bits_msb(ca_bits), info
+
+
+def encode_document(q: torch.Tensor, k: torch.Tensor, head: int, tile: int, gran: int, alpha: float = 1e-3,
+                    beta: float = 1e-2, gamma: float = 0.1, scale: Optional[float] = None):
+    """q [L, Hq, d], k [L, Hkv, d] of one document; returns (la_vec, ca_vec, info) for q-head `head`."""
+    kvh = kv_head_of(head, q.shape[1], k.shape[1])
+    p = document_probabilities(q[:, head, :], k[:, kvh, :], scale)
+    la, ca, info = encode_from_probabilities(p, tile, gran, alpha, beta, gamma)
+    info["p"] = p
+    return la, ca, info

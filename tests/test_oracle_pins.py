@@ -345,3 +345,65 @@ def test_marked_pairs_counts():
     la, ca = so.head_vectors(w, 0, 0)
     n = 90
     assert so.marked_pairs(w.shape.doc_offsets, 10, 16, 1, la, ca) == n * (n + 1) // 2
+
+
+# ------------------------------------------------------------------ Part 4: offline metadata generation (encoder)
+
+def test_encoder_uniform_attention_closed_form():
+    """q = 0 => p[q, k] = 1/(q+1) for k <= q.  LA tile (i, j) holds max p = 1/(i*T+1), so it is marked iff
+    i*T + 1 <= 1/alpha; key k is hit by rows k .. floor(1/beta)-1, so hits(k) = max(0, min(L, floor(1/beta)) - k)
+    and its bit is hits > gamma * (L - k)."""
+    n, t, d = 40, 8, 16
+    q = torch.zeros((n, 1, d), dtype=torch.bfloat16)
+    k = torch.randn((n, 1, d), generator=torch.Generator().manual_seed(1)).to(torch.bfloat16)
+    alpha, beta, gamma = 1.0 / 17.5, 1.0 / 12.5, 0.25
+    la, ca, info = so.encode_document(q, k, 0, t, 1, alpha, beta, gamma)
+    pt = 5
+    exp_la = [1 if i * t + 1 <= 17 else 0 for i in range(pt) for j in range(i + 1)]
+    assert list(info["la_bits"]) == exp_la
+    assert np.array_equal(la, so.pack_bits_msb(exp_la)) and len(la) == so.la_vector_bytes(pt)
+    exp_hits = [max(0, 12 - kk) for kk in range(n)]
+    assert list(info["hits"]) == exp_hits
+    exp_ca = [1 if exp_hits[kk] > 0.25 * (n - kk) else 0 for kk in range(n)]
+    assert list(info["ca_bits"]) == exp_ca and np.array_equal(ca, so.pack_bits_msb(exp_ca))
+    # page-granular: the same hits and cells summed over the T keys of a page
+    la2, ca2, info2 = so.encode_document(q, k, 0, t, t, alpha, beta, gamma)
+    exp_pg = []
+    for g in range(pt):
+        hits = sum(exp_hits[g * t:(g + 1) * t]); cells = sum(n - kk for kk in range(g * t, (g + 1) * t))
+        exp_pg.append(1 if hits > 0.25 * cells else 0)
+    assert list(info2["ca_bits"]) == exp_pg and len(ca2) == so.ca_vector_bytes(n, t, t) and np.array_equal(la2, la)
+
+
+def test_encoder_one_hot_attention_gives_diagonal_A4():
+    """Every row attends (almost) only to itself: only diagonal tiles hold a probability >= alpha, which for P = 3 is
+    the byte 0xA4 of the enumeration printed at PAPER.md:L203; each key is hit by exactly one row (itself)."""
+    n, t, d = 12, 4, 16
+    e = torch.eye(n, d) * 40.0                 # logits 40*40/4 = 400 on the diagonal, 0 elsewhere
+    q = e.reshape(n, 1, d).to(torch.bfloat16)
+    k = e.reshape(n, 1, d).to(torch.bfloat16)
+    la, ca, info = so.encode_document(q, k, 0, t, 1, 1e-3, 1e-2, 0.1)
+    assert bytes(la) == bytes([0xA4])
+    assert list(info["hits"]) == [1] * n
+    assert list(info["ca_bits"]) == [1 if 1 > float(np.float32(0.1)) * (n - kk) else 0 for kk in range(n)]   # the last 9 keys
+
+
+def test_encoder_thresholds_monotone_and_extremes():
+    """alpha below every causal probability marks all tiles (FF..-style all-ones vector); alpha > 1 marks none; raising
+    alpha / beta never sets a bit that was clear."""
+    n, t, d = 50, 16, 32
+    g = torch.Generator().manual_seed(3)
+    q = torch.randn((n, 2, d), generator=g).to(torch.bfloat16)
+    k = torch.randn((n, 1, d), generator=g).to(torch.bfloat16)
+    _, _, info = so.encode_document(q, k, 1, t, 1, 1e-30, 1e-30, 0.0)
+    assert info["la_bits"].all() and info["ca_bits"].all()
+    _, _, info = so.encode_document(q, k, 1, t, 1, 1.5, 1.5, 0.0)
+    assert not info["la_bits"].any() and not info["ca_bits"].any()
+    prev_la, prev_ca = None, None
+    for a in (1e-4, 1e-3, 1e-2, 1e-1):
+        _, _, info = so.encode_document(q, k, 1, t, 1, a, a, 0.1)
+        if prev_la is not None:
+            assert (info["la_bits"] <= prev_la).all() and (info["ca_bits"] <= prev_ca).all()
+        prev_la, prev_ca = info["la_bits"], info["ca_bits"]
+    # rows sum to one and the first row is the single cell p[0, 0] = 1
+    assert np.allclose(info["p"].sum(axis=1), 1.0) and info["p"][0, 0] == 1.0
