@@ -112,6 +112,25 @@ int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, int32_t n_k
                                 int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
                                 void* O, int64_t o_row_stride, float* lse, float softmax_scale, void* stream);
 
+/* ---- offline metadata generation (sec 4.1, L209 sec 4.2, L223 sec 4.4) ----
+ * Produces the LA / CA bit vectors of ONE document for the q-heads of one layer from the document's standalone dense
+ * causal attention ("SIFT is created offline by performing dense prefill on each RAG document").
+ *   LA bit (i, j) = 1 iff tile (i, j) of the document holds at least one probability >= alpha      (L201)
+ *   CA bit g      = 1 iff (cells of key group g with probability >= beta) > gamma * (causal cells of key group g);
+ *                   a key group is one key token (cross_gran = 1; "Key tokens with >10% concentration
+ *                   of high scores") or a page of `tile` keys (cross_gran = tile; L209).  DESIGN.md reading R6.
+ * Q [doc_len][n_q_heads][head_dim], K [doc_len][n_kv_heads][head_dim] bf16 dev (the document's rows only), row
+ * strides in elements; lse [n_q_heads][doc_len] fp32 dev = the natural-log row log-sum-exp of the document's dense
+ * causal attention with the same softmax_scale, e.g. from sift_dense_causal_attention on the same Q, K.
+ * la_out [n_q_heads][ceil(P(P+1)/16)], ca_out [n_q_heads][ceil(ceil(doc_len/cross_gran)/8)] dev, MSB-first, padding
+ * bits 0: the [q_head][bytes] slice of a document's blob for one layer.  workspace: dev, 16-byte aligned,
+ * >= sift_encode_workspace_size() bytes (per-key counters and per-tile flags; cleared by the call). */
+int sift_encode_workspace_size(int32_t doc_len, int32_t n_q_heads, int32_t tile, size_t* bytes);
+int sift_encode_document(int32_t doc_len, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, int32_t tile,
+                         int32_t cross_gran, const void* Q, const void* K, int64_t q_row_stride, int64_t k_row_stride,
+                         const float* lse, float alpha, float beta, float gamma, float softmax_scale,
+                         uint8_t* la_out, uint8_t* ca_out, void* workspace, size_t workspace_bytes, void* stream);
+
 /* Number of kernels the library has launched in this process (bench.py's gpu_launches). */
 int64_t sift_launch_count(void);
 

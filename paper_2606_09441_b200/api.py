@@ -14,7 +14,8 @@ from .build import LIB
 
 SIFT_OK = 0
 EXPORTS = ("sift_version", "sift_last_error", "sift_metadata_size", "sift_metadata_layout",
-           "sift_decode_metadata", "sift_prefill_attention", "sift_dense_causal_attention", "sift_launch_count")
+           "sift_decode_metadata", "sift_prefill_attention", "sift_dense_causal_attention", "sift_launch_count",
+           "sift_encode_workspace_size", "sift_encode_document")
 
 
 class SiftShape(C.Structure):
@@ -59,6 +60,10 @@ def lib() -> C.CDLL:
         L.sift_dense_causal_attention.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
                                                   C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_int64,
                                                   C.c_void_p, C.c_float, C.c_void_p]
+        L.sift_encode_workspace_size.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]
+        L.sift_encode_document.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p,
+                                           C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_float, C.c_float, C.c_float,
+                                           C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         _lib = L
     return _lib
 
@@ -199,3 +204,26 @@ def metadata_views(shape: Shape, metadata: torch.Tensor) -> Dict[str, torch.Tens
         "mblock_tile0": v(lay.mblock_tile0, lay.n_mblocks + 1), "sched": v(lay.sched, L, lay.n_items),
         "counters": v(lay.counters, L, 2),
     }
+
+
+def sift_encode_document(q: torch.Tensor, k: torch.Tensor, lse: torch.Tensor, tile: int, cross_gran: int = 1,
+                         alpha: float = 1e-3, beta: float = 1e-2, gamma: float = 0.1, softmax_scale: float = 0.0,
+                         stream=None) -> Tuple[torch.Tensor, torch.Tensor]:
+    """Offline metadata generation for one document and layer (include/sift.h).  q [L,Hq,d], k [L,Hkv,d] bf16 CUDA,
+    lse [Hq,L] fp32 CUDA (from sift_dense_causal_attention on the document).  Returns (la [Hq, la_bytes], ca [Hq, ca_bytes])."""
+    assert q.is_cuda and k.is_cuda and lse.is_cuda and q.dtype == torch.bfloat16 and k.dtype == torch.bfloat16
+    assert lse.dtype == torch.float32 and lse.is_contiguous() and q.stride(2) == 1 and k.stride(2) == 1
+    assert q.stride(1) == q.shape[2] and k.stride(1) == k.shape[2]
+    n, hq, d = q.shape
+    hkv = k.shape[1]
+    pt = -(-n // tile)
+    la_bytes, ca_bytes = -(-(pt * (pt + 1) // 2) // 8), -(-(-(-n // cross_gran)) // 8)
+    nb = C.c_size_t()
+    _check(lib().sift_encode_workspace_size(n, hq, tile, C.byref(nb)), "sift_encode_workspace_size")
+    ws = torch.empty(nb.value, dtype=torch.uint8, device=q.device)
+    la = torch.empty((hq, la_bytes), dtype=torch.uint8, device=q.device)
+    ca = torch.empty((hq, ca_bytes), dtype=torch.uint8, device=q.device)
+    _check(lib().sift_encode_document(n, hq, hkv, d, tile, cross_gran, q.data_ptr(), k.data_ptr(), q.stride(0), k.stride(0),
+                                      lse.data_ptr(), alpha, beta, gamma, softmax_scale, la.data_ptr(), ca.data_ptr(),
+                                      ws.data_ptr(), nb.value, _stream(stream)), "sift_encode_document")
+    return la, ca

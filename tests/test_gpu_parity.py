@@ -4,6 +4,7 @@ import pytest
 import torch
 
 from paper_2606_09441_b200 import api, workload as wl
+from oracle import sift_oracle as so
 from tests import gpu_util as gu
 
 pytestmark = pytest.mark.gpu
@@ -184,3 +185,101 @@ def test_repeat_calls_share_metadata():
     o2, l2 = api.sift_prefill_attention(shape, 0, q, k, v, md)
     torch.cuda.synchronize()
     assert torch.equal(o1, o2) and torch.equal(l1, l2)
+
+
+# ------------------------------------------------------------------ offline metadata generation
+
+def _unpack(vec, nbits):
+    return np.unpackbits(np.asarray(vec, dtype=np.uint8), bitorder="big")[:nbits]
+
+
+def _encode_case(n, hq, hkv, d, tile, gran, seed, alpha=1e-3, beta=1e-2, gamma=0.1, q_gain=1.0):
+    """GPU encoder vs oracle on one synthetic document.  A floating-point score decides each bit; the GPU works from
+    bf16 tensor-core dot products in fp32 and an fp32 LSE, the oracle in fp64, so cells whose probability lies within
+    REL of a threshold may legitimately fall on either side: a bit is compared only when no such cell can change it
+    (both sides take the decision on p >= threshold)."""
+    REL = 2e-3
+    g = torch.Generator().manual_seed(seed)
+    q = (torch.randn((n, hq, d), generator=g) * q_gain).to(torch.bfloat16)
+    k = torch.randn((n, hkv, d), generator=g).to(torch.bfloat16)
+    v = torch.randn((n, hkv, d), generator=g).to(torch.bfloat16)
+    qc, kc, vc = q.cuda(), k.cuda(), v.cuda()
+    _, lse = api.sift_dense_causal_attention(qc, kc, vc)            # pass 1: row log-sum-exp of the document
+    la, ca = api.sift_encode_document(qc, kc, lse, tile, gran, alpha, beta, gamma)
+    torch.cuda.synchronize()
+    la, ca = la.cpu().numpy(), ca.cpu().numpy()
+    pt = -(-n // tile)
+    n_la, n_ca = pt * (pt + 1) // 2, -(-n // gran)
+    checked = skipped = 0
+    for h in range(hq):
+        la_o, ca_o, info = so.encode_document(q, k, h, tile, gran, alpha, beta, gamma)
+        assert la.shape[1] == len(la_o) and ca.shape[1] == len(ca_o)
+        p = info["p"]
+        # padding bits must be zero
+        assert not np.unpackbits(la[h], bitorder="big")[n_la:].any() and not np.unpackbits(ca[h], bitorder="big")[n_ca:].any()
+        got_la, got_ca = _unpack(la[h], n_la), _unpack(ca[h], n_ca)
+        sure = np.abs(info["la_max"] / alpha - 1.0) > REL
+        assert np.array_equal(got_la[sure], info["la_bits"][sure]), (h, "LA")
+        checked += int(sure.sum()); skipped += int((~sure).sum())
+        near = ((np.abs(p / beta - 1.0) <= REL) & np.tril(np.ones(p.shape, dtype=bool))).sum(axis=0)   # per key column
+        g32 = float(np.float32(gamma))
+        for gi in range(n_ca):
+            ks = slice(gi * gran, min(n, (gi + 1) * gran))
+            amb = int(near[ks].sum())
+            lo, hi = info["hits"][gi] - amb, info["hits"][gi] + amb
+            thr = g32 * info["cells"][gi]
+            if (lo > thr) == (hi > thr):
+                assert got_ca[gi] == info["ca_bits"][gi], (h, "CA", gi)
+                checked += 1
+            else:
+                skipped += 1
+    print(f"[encode] n={n} T={tile} G={gran}: {checked} bits compared, {skipped} on a threshold (not compared)")
+    assert skipped <= 0.02 * (checked + skipped) + 2
+    return checked
+
+
+@pytest.mark.parametrize("case", [
+    dict(n=300, hq=2, hkv=1, d=128, tile=128, gran=1, seed=1),
+    dict(n=1000, hq=4, hkv=2, d=128, tile=128, gran=1, seed=2, q_gain=2.0),
+    dict(n=700, hq=2, hkv=2, d=64, tile=64, gran=1, seed=3, q_gain=1.5),
+    dict(n=1000, hq=2, hkv=1, d=128, tile=128, gran=128, seed=4, q_gain=2.0),
+    dict(n=333, hq=3, hkv=3, d=64, tile=64, gran=64, seed=5, q_gain=3.0),
+    dict(n=1, hq=1, hkv=1, d=64, tile=64, gran=1, seed=6),
+])
+def test_encode_document_matches_oracle(case):
+    assert _encode_case(**case) > 0
+
+
+def test_encode_then_decode_then_attend_round_trip():
+    """The vectors the encoder writes are consumed by the decoder and the attention kernel: two documents encoded from
+    their own Q/K, placed in a prompt, decoded, attended; output compared with the oracle driven by the SAME vectors."""
+    lens, hq, hkv, d, tile = (640, 500), 2, 1, 128, 128
+    w = wl.custom("enc-rt", n_q_heads=hq, n_kv_heads=hkv, head_dim=d, doc_lens=lens, query_len=100, tile=tile, seed=7)
+    q, k, v = w.qkv(0)
+    q = (q.float() * 2.0).to(torch.bfloat16)
+    la_parts, ca_parts, la_off, ca_off = [], [], [], []
+    pos_la = pos_ca = 0
+    off = [int(x) for x in w.shape.doc_offsets]
+    for dd in range(2):
+        qd, kd, vd = (t[off[dd]:off[dd + 1]].contiguous().cuda() for t in (q, k, v))
+        _, lse = api.sift_dense_causal_attention(qd, kd, vd)
+        la, ca = api.sift_encode_document(qd, kd, lse, tile, 1)
+        la_off.append(pos_la); ca_off.append(pos_ca)
+        la_parts.append(la.cpu().numpy().reshape(-1)); ca_parts.append(ca.cpu().numpy().reshape(-1))
+        pos_la += la_parts[-1].size; pos_ca += ca_parts[-1].size
+    from dataclasses import replace
+    w2 = replace(w, la_blob=np.concatenate(la_parts + [np.zeros(16, np.uint8)]), ca_blob=np.concatenate(ca_parts + [np.zeros(16, np.uint8)]),
+                 la_doc_off=np.array(la_off, np.int64), ca_doc_off=np.array(ca_off, np.int64))
+    shape, md = gu.decode_on_gpu(w2)
+    gu.assert_metadata_equal(w2, shape, md)
+    o, lse = api.sift_prefill_attention(shape, 0, q.cuda(), k.cuda(), v.cuda(), md)
+    torch.cuda.synchronize()
+    sh = w2.shape
+    mx = 0.0
+    for h in range(hq):
+        la_v, ca_v = so.head_vectors(w2, 0, h)
+        rows = list(range(0, sh.n_tokens, 7))
+        oo, ll = so.sift_attention_rows(q, k, v, h, sh.doc_offsets, sh.query_len, sh.tile, sh.cross_gran, la_v, ca_v, rows)
+        mx = max(mx, float((o.float().cpu()[rows, h, :] - oo).abs().max()))
+        assert float((lse.cpu()[h, rows] - ll).abs().max()) <= gu.TOL_LSE
+    assert mx <= gu.TOL_MAX
