@@ -271,6 +271,16 @@ def run_ours(args):
              "speedup_vs_dense": den_ms / att_ms, "marked_density": case.flops / case.dense_flops,
              "decode_GBps": case.decode_bytes / (dec_ms * 1e-3) / 1e9, "decode_bytes": case.decode_bytes,
              "frac_of_sustained_peak": achieved / peaks["bf16_sustained"], "n_tokens": w.shape.n_tokens}
+    if args.config == "32k" and world == 1:
+        # offline metadata generation for one 2000-token document of this prompt and layer: pass 1 =
+        # dense causal attention of the document alone (row LSE), pass 2 = sift_encode_document
+        n0 = int(w.shape.doc_offsets[1])
+        qd, kd, vd = case.q[:n0], case.k[:n0], case.v[:n0]
+        od, lsed = api.sift_dense_causal_attention(qd, kd, vd)
+        enc = float(np.median(time_each(lambda: api.sift_encode_document(qd, kd, lsed, w.shape.tile, 1), 10)))
+        p1 = float(np.median(time_each(lambda: api.sift_dense_causal_attention(qd, kd, vd, od, lsed), 10)))
+        extra["encode"] = {"doc_tokens": n0, "pass1_dense_lse_us": p1 * 1e3, "pass2_encode_us": enc * 1e3,
+                           "qk_tflops": 2 * w.shape.head_dim * w.shape.n_q_heads * n0 * (n0 + 1) // 2 / (enc * 1e-3) / 1e12}
     if args.with_64k and args.config == "32k" and world == 1:
         c4 = GpuCase(wl.config_64k_ragged(seed))
         for _ in range(3):

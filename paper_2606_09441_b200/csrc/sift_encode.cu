@@ -134,13 +134,16 @@ sift_encode_scores_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid
         wb |= (valid && x >= p.log2_beta) ? (1u << cc) : 0u;
       }
       any_a[c >> 1] = any_a[c >> 1] || aa;
-      // per-key counts of this warp's 32 rows: ballot over the rows, one column at a time
-      int cnt = 0;
+      // per-key counts of this warp's 32 rows: transpose the 32 x 32 bit matrix (lane = row, bit = column) with five
+      // butterfly exchanges so that lane c holds column c, then popc (5 shuffles instead of 32 ballots)
+      uint32_t xt = wb;
 #pragma unroll
-      for (int cc = 0; cc < 32; ++cc) {
-        const uint32_t b = __ballot_sync(0xffffffffu, (wb >> cc) & 1u);
-        if (lane == cc) cnt = __popc(b);
+      for (int jj = 16; jj >= 1; jj >>= 1) {
+        const uint32_t mk = (jj == 16) ? 0x0000ffffu : (jj == 8) ? 0x00ff00ffu : (jj == 4) ? 0x0f0f0f0fu : (jj == 2) ? 0x33333333u : 0x55555555u;
+        const uint32_t y = __shfl_xor_sync(0xffffffffu, xt, jj);
+        xt = (lane & jj) ? ((xt & ~mk) | ((y >> jj) & mk)) : ((xt & mk) | ((y << jj) & ~mk));
       }
+      const int cnt = __popc(xt);
       if (cnt) atomicAdd(&p.col_cnt[(int64_t)h * p.len128 + key0 + c * 32 + lane], cnt);
     }
     if (T == 64) {
