@@ -128,6 +128,7 @@ class GpuCase:
         self.o = torch.empty_like(self.q)
         self.lse = torch.empty((q.shape[1], q.shape[0]), dtype=torch.float32, device="cuda")
         self.o_h = torch.empty(self.o.shape, dtype=self.o.dtype).pin_memory()
+        self.pipe = None
         self.decode()
         torch.cuda.synchronize()
         views = {k_: t.cpu().numpy() for k_, t in api.metadata_views(self.shape, self.md).items()}
@@ -151,14 +152,13 @@ class GpuCase:
         self.attention()
 
     def e2e_step(self):
-        """Same step through the public API with HOST buffers: H2D of bit vectors and Q/K/V, D2H of O."""
-        self.la.copy_(self.la_h, non_blocking=True)
-        self.ca.copy_(self.ca_h, non_blocking=True)
-        self.q.copy_(self.q_h, non_blocking=True)
-        self.k.copy_(self.k_h, non_blocking=True)
-        self.v.copy_(self.v_h, non_blocking=True)
-        self.step()
-        self.o_h.copy_(self.o, non_blocking=True)
+        """Same step with HOST buffers (pinned): H2D of bit vectors and Q/K/V, decode + attention, D2H of O, through
+        paper_2606_09441_b200.pipeline (per kv-head group, copies in both directions overlapped with the kernels)."""
+        if self.pipe is None:
+            from paper_2606_09441_b200.pipeline import HostLayerPipeline
+            self.pipe = HostLayerPipeline(self.w.shape)
+        self.pipe.run(self.la_h, self.ca_h, self.w.la_doc_off, self.w.ca_doc_off, self.q_h, self.k_h, self.v_h, self.o_h,
+                      self.layer)
 
     @property
     def h2d_bytes(self):

@@ -283,3 +283,21 @@ def test_encode_then_decode_then_attend_round_trip():
         mx = max(mx, float((o.float().cpu()[rows, h, :] - oo).abs().max()))
         assert float((lse.cpu()[h, rows] - ll).abs().max()) <= gu.TOL_LSE
     assert mx <= gu.TOL_MAX
+
+
+def test_host_pipeline_matches_single_call():
+    """The host-buffer pipeline (per kv-head group, three streams) must give exactly what one call over all heads gives."""
+    from paper_2606_09441_b200.pipeline import HostLayerPipeline
+    w = wl.custom("pipe", n_q_heads=8, n_kv_heads=4, head_dim=128, doc_lens=(700, 300, 520), query_len=90, tile=128,
+                  p_cross=0.4, seed=31)
+    _, _, o_ref, lse_ref = gu.run_sift(w)
+    q, k, v = (t.pin_memory() for t in w.qkv(0))
+    la_h, ca_h = torch.from_numpy(w.la_blob).pin_memory(), torch.from_numpy(w.ca_blob).pin_memory()
+    o_h = torch.empty(q.shape, dtype=q.dtype).pin_memory()
+    pipe = HostLayerPipeline(w.shape)
+    for _ in range(2):                       # twice: buffers and metadata are reused across calls
+        o_h.zero_()
+        pipe.run(la_h, ca_h, w.la_doc_off, w.ca_doc_off, q, k, v, o_h)
+        pipe.wait()
+        assert torch.equal(o_h, o_ref.cpu())
+    assert torch.equal(pipe.lse.cpu(), lse_ref.cpu())
