@@ -43,9 +43,6 @@ constexpr int kFirstVWarp = 4 + 4 * kNQ;
 constexpr int kProducerThreads = 96;              // per operand: K = warps 2, 3, 14; V = warps 12, 13, 15
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 with a stale max
 constexpr uint32_t kTmemCols = 512;
-#ifndef SIFT_SM_V2
-#define SIFT_SM_V2 0
-#endif
 #ifndef SIFT_EXP_EMU_MASK
 #define SIFT_EXP_EMU_MASK 0x0
 #endif
@@ -587,17 +584,6 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
           for (int c = 0; c < kBN; ++c) s[c] = (c < cur_lim) ? s[c] : -INFINITY;
         }
-#if SIFT_SM_V2 & 1
-        float mx8[8];                                              // eight independent chains of 3-input max
-#pragma unroll
-        for (int j = 0; j < 8; ++j) mx8[j] = fmaxf(s[2 * j], s[2 * j + 1]);
-#pragma unroll
-        for (int c = 16; c < kBN; c += 16) {
-#pragma unroll
-          for (int j = 0; j < 8; ++j) mx8[j] = fmaxf(mx8[j], fmaxf(s[c + 2 * j], s[c + 2 * j + 1]));
-        }
-        const float mx = fmaxf(fmaxf(fmaxf(mx8[0], mx8[1]), fmaxf(mx8[2], mx8[3])), fmaxf(fmaxf(mx8[4], mx8[5]), fmaxf(mx8[6], mx8[7])));
-#else
         float mx4[4] = {s[0], s[1], s[2], s[3]};                  // four independent chains
 #pragma unroll
         for (int c = 4; c < kBN; c += 4) {
@@ -605,7 +591,6 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           mx4[2] = fmaxf(mx4[2], s[c + 2]); mx4[3] = fmaxf(mx4[3], s[c + 3]);
         }
         const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
-#endif
         const float m_new = fmaxf(m, mx);
         const bool need = (m_new - m) * sl > kRescaleThreshold;   // (-inf) - (-inf) = NaN -> false
         if (__any_sync(0xffffffffu, need)) {
@@ -633,21 +618,10 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
         for (int c = 0; c < kBN / 32; ++c) {
           uint32_t pk[16];
-          float2 xq[2];
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
-#if SIFT_SM_V2 & 2
-            // x of pair i+2 is issued (volatile order) before the two ex2 of pair i: the FMA-pipe work rides in the
-            // issue slots the 8-clk MUFU instructions leave free
-            if (i == 0) { xq[0] = fma2v(make_float2(s[c * 32], s[c * 32 + 1]), sl2, nm2); xq[1] = fma2v(make_float2(s[c * 32 + 2], s[c * 32 + 3]), sl2, nm2); }
-            const float2 x = xq[i & 1];
-            if (i + 2 < 16) xq[i & 1] = fma2v(make_float2(s[c * 32 + 2 * i + 4], s[c * 32 + 2 * i + 5]), sl2, nm2);
-            float2 pr;
-            if (true) { pr = make_float2(ex2v(x.x), ex2v(x.y)); } else
-#else
             const float2 x = fma2(make_float2(s[c * 32 + 2 * i], s[c * 32 + 2 * i + 1]), sl2, nm2);
             float2 pr;
-#endif
             if ((kExpEmuMask >> (i & 3)) & 1) {
               pr = ex2_poly2(x);                 // this pair on the FMA pipe: the MUFU is the co-bottleneck (DESIGN 5.2)
             } else {

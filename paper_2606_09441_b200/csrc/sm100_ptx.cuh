@@ -210,23 +210,6 @@ __device__ __forceinline__ float2 add2(float2 a, float2 b) {
   asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
   return d;
 }
-// volatile twins: used where the program order of FMA-pipe and MUFU instructions should survive scheduling
-__device__ __forceinline__ float2 fma2v(float2 a, float2 b, float2 c) {
-  uint64_t ra, rb, rc, rd;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
-  asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
-  asm("mov.b64 %0, {%1, %2};" : "=l"(rc) : "f"(c.x), "f"(c.y));
-  asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
-  float2 d;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
-  return d;
-}
-__device__ __forceinline__ float ex2v(float x) {
-  float y;
-  asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-
 // 2^x for a pair on the FMA/ALU pipes instead of the MUFU: round-to-nearest split x = n + f (magic-number add),
 // cubic minimax polynomial for 2^f on [-0.5, 0.5] (max relative error 7.5e-5, far below the bf16 rounding of P),
 // exponent patched in with an integer add.  x is clamped at -126 (masked entries are -inf -> ~1e-38 ~ 0).
