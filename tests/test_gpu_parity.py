@@ -301,3 +301,34 @@ def test_host_pipeline_matches_single_call():
         pipe.wait()
         assert torch.equal(o_h, o_ref.cpu())
     assert torch.equal(pipe.lse.cpu(), lse_ref.cpu())
+
+
+def test_no_out_of_bounds_writes_guard_bands():
+    """Outputs sit between guard bands (compute-sanitizer is not available on the GPU pool): metadata, O and LSE of a
+    ragged prompt with non-tile-multiple lengths; the bands must come back untouched."""
+    w = wl.custom("guard", n_q_heads=4, n_kv_heads=2, head_dim=128, doc_lens=(130, 257, 1, 640, 77), query_len=61,
+                  tile=128, p_cross=0.5, seed=37)
+    shape = api.Shape.from_prompt(w.shape)
+    G = 4096
+    nb = api.sift_metadata_size(shape)
+    md_all = torch.full((nb + 2 * G,), 0xAB, dtype=torch.uint8, device="cuda")
+    md = md_all[G:G + nb]
+    la, ca = torch.from_numpy(w.la_blob).cuda(), torch.from_numpy(w.ca_blob).cuda()
+    api.sift_decode_metadata(shape, la, w.la_doc_off, ca, w.ca_doc_off, md)
+    q, k, v = (t.cuda() for t in w.qkv(0))
+    n, hq, d = q.shape
+    o_all = torch.full((n * hq * d + 2 * G,), -7.0, dtype=torch.bfloat16, device="cuda")
+    o = o_all[G:G + n * hq * d].view(n, hq, d)
+    lse_all = torch.full((hq * n + 2 * G,), -7.0, dtype=torch.float32, device="cuda")
+    lse = lse_all[G:G + hq * n].view(hq, n)
+    api.sift_prefill_attention(shape, 0, q, k, v, md, o, lse)
+    api.sift_dense_causal_attention(q, k, v, o, lse)
+    torch.cuda.synchronize()
+    assert bool((md_all[:G] == 0xAB).all()) and bool((md_all[G + nb:] == 0xAB).all())
+    assert bool((o_all[:G] == -7.0).all()) and bool((o_all[G + n * hq * d:] == -7.0).all())
+    assert bool((lse_all[:G] == -7.0).all()) and bool((lse_all[G + hq * n:] == -7.0).all())
+    gu.assert_metadata_equal(w, shape, md)
+    # encoder outputs and workspace
+    la_o, ca_o = api.sift_encode_document(q[:130].contiguous(), k[:130].contiguous(), lse[:, :130].contiguous(), 128, 1)
+    torch.cuda.synchronize()
+    assert la_o.shape == (hq, 1) and ca_o.shape == (hq, 17)
