@@ -1,0 +1,107 @@
+/* Plain-C client of include/sift.h (no Python, no torch): proves the boundary is a C ABI.
+ *   abi_smoke host   -> host-only calls: version, layout arithmetic, error codes        (runs without a GPU)
+ *   abi_smoke gpu    -> decode + dense/sparse attention on a small prompt through cudaMalloc'd buffers
+ * Expected values are closed forms: all-ones bit vectors => counts are sizes; Q = 0 => uniform attention, so every
+ * output row is the running mean of the V rows it may see, and LSE = ln(#keys). */
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "sift.h"
+
+#define CHECK(c) do { if (!(c)) { fprintf(stderr, "FAILED %s:%d: %s (last error: %s)\n", __FILE__, __LINE__, #c, sift_last_error()); return 1; } } while (0)
+
+/* minimal CUDA runtime prototypes (the test links libcudart but needs no CUDA headers) */
+extern int cudaMalloc(void** p, size_t n);
+extern int cudaMemcpy(void* dst, const void* src, size_t n, int kind);
+extern int cudaMemset(void* p, int v, size_t n);
+extern int cudaDeviceSynchronize(void);
+extern int cudaFree(void* p);
+
+static uint16_t f2bf(float f) { uint32_t u; memcpy(&u, &f, 4); u += 0x7fffu + ((u >> 16) & 1u); return (uint16_t)(u >> 16); }
+static float bf2f(uint16_t h) { uint32_t u = (uint32_t)h << 16; float f; memcpy(&f, &u, 4); return f; }
+
+static int host_part(void) {
+  int32_t off[3] = {0, 300, 500};
+  sift_shape s = {sizeof(sift_shape), 2, 4, 2, 128, 2, 70, 128, 1, off};
+  sift_md_layout lay;
+  size_t nb = 0;
+  CHECK(strstr(sift_version(), "sift-b200") != NULL);
+  CHECK(sift_metadata_layout(&s, &lay) == SIFT_OK);
+  CHECK(sift_metadata_size(&s, &nb) == SIFT_OK && nb == lay.total_bytes);
+  CHECK(lay.n_tiles == 3 + 2 + 1);                       /* ceil(300/128) + ceil(200/128) + ceil(70/128) */
+  CHECK(lay.cross_cap == 512);                           /* 500 key bits rounded up to 128 */
+  CHECK(lay.local_cap == 6 + 3 + 6);                     /* 3*4/2 + 2*3/2 + (query tile with global id 5: 6 entries) */
+  s.head_dim = 96;
+  CHECK(sift_metadata_size(&s, &nb) == SIFT_ERR_UNSUPPORTED && strlen(sift_last_error()) > 0);
+  s.head_dim = 128; off[2] = 300;
+  CHECK(sift_metadata_size(&s, &nb) == SIFT_ERR_INVALID_ARG);
+  CHECK(sift_metadata_size(NULL, &nb) == SIFT_ERR_INVALID_ARG);
+  CHECK(sift_encode_workspace_size(300, 4, 128, &nb) == SIFT_OK && nb == 4u * (384u + 6u) * 4u);
+  printf("abi_smoke host ok\n");
+  return 0;
+}
+
+static int gpu_part(void) {
+  enum { L0 = 200, L1 = 150, LQ = 34, N = L0 + L1 + LQ, HQ = 2, HKV = 1, D = 64, T = 64 };
+  int32_t off[3] = {0, L0, L0 + L1};
+  sift_shape s = {sizeof(sift_shape), 1, HQ, HKV, D, 2, LQ, T, 1, off};
+  sift_md_layout lay;
+  CHECK(sift_metadata_layout(&s, &lay) == SIFT_OK);
+  /* all-ones vectors: per document [layer][head][bytes]; P = 4 and 3 -> LA 10 / 6 bits -> 2 / 1 bytes; CA 25 / 19 bytes */
+  const int la_b[2] = {2, 1}, ca_b[2] = {25, 19};
+  uint8_t la[HQ * 3 + 16], ca[HQ * 44 + 16];
+  memset(la, 0xff, sizeof(la)); memset(ca, 0xff, sizeof(ca));
+  int64_t la_off[2] = {0, HQ * la_b[0]}, ca_off[2] = {0, HQ * ca_b[0]};
+  void *d_la, *d_ca, *d_md, *d_q, *d_k, *d_v, *d_o, *d_lse;
+  CHECK(cudaMalloc(&d_la, sizeof(la)) == 0 && cudaMalloc(&d_ca, sizeof(ca)) == 0 && cudaMalloc(&d_md, lay.total_bytes) == 0);
+  CHECK(cudaMemcpy(d_la, la, sizeof(la), 1) == 0 && cudaMemcpy(d_ca, ca, sizeof(ca), 1) == 0);
+  CHECK(sift_decode_metadata(&s, (const uint8_t*)d_la, la_off, (const uint8_t*)d_ca, ca_off, d_md, lay.total_bytes, NULL) == SIFT_OK);
+  int32_t* md = (int32_t*)malloc(lay.total_bytes);
+  CHECK(cudaDeviceSynchronize() == 0 && cudaMemcpy(md, d_md, lay.total_bytes, 2) == 0);
+  const int32_t* cross_ptr = (const int32_t*)((const char*)md + lay.cross_ptr);
+  const int32_t* local_ptr = (const int32_t*)((const char*)md + lay.local_ptr);
+  const int32_t* cross_idx = (const int32_t*)((const char*)md + lay.cross_idx);
+  for (int h = 0; h < HQ; ++h) {
+    CHECK(cross_ptr[h * 3 + 0] == 0 && cross_ptr[h * 3 + 1] == L0 && cross_ptr[h * 3 + 2] == L0 + L1);   /* padding bits ignored */
+    CHECK(local_ptr[h * (lay.n_tiles + 1) + lay.n_tiles] == 10 + 6 + 8);                                  /* + query tile id 7: 8 entries */
+    for (int i = 0; i < L0 + L1; ++i) CHECK(cross_idx[(size_t)h * lay.cross_cap + i] == i);
+  }
+  /* Q = 0, K arbitrary, V[n][c] = n (exact in bf16 up to 256; use n mod 64): all bits set => dense causal attention */
+  uint16_t* hq = (uint16_t*)calloc((size_t)N * HQ * D, 2);
+  uint16_t* hk = (uint16_t*)malloc((size_t)N * HKV * D * 2);
+  uint16_t* hv = (uint16_t*)malloc((size_t)N * HKV * D * 2);
+  for (int n = 0; n < N; ++n) for (int c = 0; c < D; ++c) { hk[n * D + c] = f2bf((float)((n * 7 + c) % 5) - 2.f); hv[n * D + c] = f2bf((float)(n % 64)); }
+  size_t qb = (size_t)N * HQ * D * 2, kb = (size_t)N * HKV * D * 2;
+  CHECK(cudaMalloc(&d_q, qb) == 0 && cudaMalloc(&d_k, kb) == 0 && cudaMalloc(&d_v, kb) == 0 && cudaMalloc(&d_o, qb) == 0 && cudaMalloc(&d_lse, (size_t)HQ * N * 4) == 0);
+  CHECK(cudaMemcpy(d_q, hq, qb, 1) == 0 && cudaMemcpy(d_k, hk, kb, 1) == 0 && cudaMemcpy(d_v, hv, kb, 1) == 0);
+  uint16_t* ho = (uint16_t*)malloc(qb);
+  float* hl = (float*)malloc((size_t)HQ * N * 4);
+  for (int pass = 0; pass < 2; ++pass) {
+    CHECK(cudaMemset(d_o, 0xff, qb) == 0);
+    int rc = pass == 0 ? sift_prefill_attention(&s, 0, d_q, d_k, d_v, HQ * D, HKV * D, HKV * D, d_md, d_o, HQ * D, (float*)d_lse, 0.f, NULL)
+                       : sift_dense_causal_attention(N, HQ, HKV, D, d_q, d_k, d_v, HQ * D, HKV * D, HKV * D, d_o, HQ * D, (float*)d_lse, 0.f, NULL);
+    CHECK(rc == SIFT_OK);
+    CHECK(cudaDeviceSynchronize() == 0 && cudaMemcpy(ho, d_o, qb, 2) == 0 && cudaMemcpy(hl, d_lse, (size_t)HQ * N * 4, 2) == 0);
+    double sum = 0;
+    for (int n = 0; n < N; ++n) {
+      sum += (double)(n % 64);
+      const double mean = sum / (n + 1);
+      for (int h = 0; h < HQ; ++h) {
+        CHECK(fabs(bf2f(ho[((size_t)n * HQ + h) * D + 5]) - mean) <= 0.02 * (1.0 + mean));
+        CHECK(fabs(hl[(size_t)h * N + n] - log((double)(n + 1))) <= 1e-3);
+      }
+    }
+  }
+  CHECK(sift_launch_count() >= 4);
+  cudaFree(d_la); cudaFree(d_ca); cudaFree(d_md); cudaFree(d_q); cudaFree(d_k); cudaFree(d_v); cudaFree(d_o); cudaFree(d_lse);
+  printf("abi_smoke gpu ok\n");
+  return 0;
+}
+
+int main(int argc, char** argv) {
+  if (argc > 1 && strcmp(argv[1], "gpu") == 0) return gpu_part();
+  return host_part();
+}
