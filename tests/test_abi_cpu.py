@@ -46,9 +46,10 @@ def test_bad_arguments_rejected():
                 tile=64)
     api.sift_metadata_size(api.Shape(**good))
     api.sift_metadata_size(api.Shape(**{**good, "cross_gran": 64}))    # page-granular CA: G = tile
+    api.sift_metadata_size(api.Shape(**{**good, "doc_offsets": np.arange(0, 513 * 8, 8)}))   # SIFT_MAX_DOCS = 512 documents
     for bad in (dict(head_dim=96), dict(tile=32), dict(cross_gran=32), dict(n_kv_heads=3),
                 dict(doc_offsets=np.array([0, 100, 100])), dict(doc_offsets=np.array([1, 100])),
-                dict(doc_offsets=np.arange(0, 64 * 600, 64))):
+                dict(doc_offsets=np.arange(0, 64 * 600, 64)), dict(doc_offsets=np.arange(0, 514 * 8, 8))):   # > SIFT_MAX_DOCS
         with pytest.raises(api.SiftError):
             api.sift_metadata_size(api.Shape(**{**good, **bad}))
     # NULL device pointers are refused before any launch

@@ -49,6 +49,20 @@ def test_decode_no_docs():
     gu.assert_metadata_equal(w, shape, md)
 
 
+def test_decode_full_stack_32_layers_launch_config():
+    """BASELINE.json configs[4] at full size: one decode call for 32 layers x 32 heads (the grid bench.py --config
+    full-stack launches); the oracle checks the first and the last layer."""
+    w = wl.config_full_stack(n_layers=32)
+    shape, md = gu.decode_on_gpu(w)
+    gu.assert_metadata_equal(w, shape, md, layers=[0, 31])
+
+
+def test_decode_max_docs():
+    w = wl.custom("maxdocs", doc_lens=tuple([5 + (i % 70) for i in range(512)]), query_len=9, tile=64, n_q_heads=2, seed=43)
+    shape, md = gu.decode_on_gpu(w)
+    gu.assert_metadata_equal(w, shape, md)
+
+
 def test_decode_full_stack_sampled_layers_and_reorder():
     w = wl.config_full_stack(n_layers=4)
     for perm in wl.stack_orderings(w, 2):
