@@ -346,3 +346,27 @@ def test_no_out_of_bounds_writes_guard_bands():
     la_o, ca_o = api.sift_encode_document(q[:130].contiguous(), k[:130].contiguous(), lse[:, :130].contiguous(), 128, 1)
     torch.cuda.synchronize()
     assert la_o.shape == (hq, 1) and ca_o.shape == (hq, 17)
+
+
+def test_randomised_shapes_and_modes(monkeypatch):
+    """30 random small prompts: head_dim, tile, GQA ratio, 0..6 documents of 1..3000 tokens, query length, CA
+    granularity, mark densities (incl. none / all), diagonal tiles forced or not, either gather mode; metadata
+    bit-exact, attention within tolerance on all rows (sampled rows above 900 tokens)."""
+    rng = np.random.default_rng(20260609)
+    for ci in range(30):
+        hd = int(rng.choice([64, 128])); tile = int(rng.choice([64, 128]))
+        hkv = int(rng.choice([1, 2, 3])); hq = hkv * int(rng.choice([1, 2, 4]))
+        nd = int(rng.integers(0, 7))
+        lens = tuple(int(x) for x in rng.integers(1, int(rng.choice([70, 700, 3000])), nd))
+        ql = int(rng.integers(0, 300)) if nd > 0 else int(rng.integers(1, 300))
+        case = dict(n_q_heads=hq, n_kv_heads=hkv, head_dim=hd, doc_lens=lens, query_len=ql, tile=tile,
+                    cross_gran=int(rng.choice([1, tile])), p_loc=float(rng.choice([-1.0, 0.1, 0.5, 1.1])),
+                    p_cross=float(rng.choice([-1.0, 0.05, 0.3, 0.9, 1.1])), diag_set=bool(rng.random() < 0.7), seed=2000 + ci)
+        monkeypatch.setenv("SIFT_GATHER_MODE", "1" if rng.random() < 0.3 else "0")
+        w = wl.custom("fuzz", **case)
+        shape, md, o, lse = gu.run_sift(w)
+        gu.assert_metadata_equal(w, shape, md)
+        n = w.shape.n_tokens
+        rows = range(n) if n <= 900 else sorted(set(int(x) for x in rng.integers(0, n, 500)) | {0, n - 1})
+        mx, mean, le = gu.attention_errors(w, 0, o, lse, range(min(hq, 4)), rows)
+        assert mx <= gu.TOL_MAX and mean <= gu.TOL_MEAN and le <= gu.TOL_LSE, (case, mx, mean, le)
