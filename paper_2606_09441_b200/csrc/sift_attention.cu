@@ -86,8 +86,10 @@ template <int HD>
 struct Smem {
   static constexpr int kHalves = HD / 64;
   static constexpr int kTileBytes = kBN * HD * 2;          // one K or V tile / one Q tile
-  static constexpr int kKStages = (kNQ == 1) ? 3 : (HD == 128 ? 3 : 4);
-  static constexpr int kVStages = (kNQ == 1) ? 3 : (HD == 128 ? 2 : 4);
+  // d = 128: 5 stages of 32 KB fit beside the two Q tiles; 2 K + 3 V measured 1-3% faster than 3 K + 2 V (a V stage is
+  // held from the P V of one step to the end of the next, a K stage only across its own Q K^T)
+  static constexpr int kKStages = (HD == 128 ? 2 : 4);
+  static constexpr int kVStages = (HD == 128 ? 3 : 4);
   static constexpr int kQOff = 0;
   static constexpr int kKOff = kQOff + kNQ * kTileBytes;
   static constexpr int kVOff = kKOff + kKStages * kTileBytes;
