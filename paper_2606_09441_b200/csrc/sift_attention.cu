@@ -49,8 +49,10 @@ constexpr uint32_t kTmemCols = 512;
 constexpr int kExpEmuMask = SIFT_EXP_EMU_MASK;   // bit j: pairs with (index & 3) == j compute 2^x by polynomial instead of MUFU.EX2
 
 constexpr int kRegsEntry = (kNQ == 2) ? 128 : 168;               // what __launch_bounds__(kNumThreads, 1) yields
-constexpr int kRegsOther = 48;                                   // non-softmax warps after setmaxnreg.dec
-constexpr int kRegsSoftmax = (kNQ == 2) ? 208 : 232;              // softmax warps after setmaxnreg.inc
+// 4 warps per sub-partition share 512 registers per lane: 2 x 216 + 2 x 40 (measured: 208/48 -1%, 200/56 -5%, 192/64 -30%:
+// the softmax loop holds a whole 128-column row of S)
+constexpr int kRegsOther = 40;                                   // non-softmax warps after setmaxnreg.dec
+constexpr int kRegsSoftmax = 216;              // softmax warps after setmaxnreg.inc
 
 static_assert(kNQ * kRegsSoftmax + 2 * kRegsOther <= (kNumThreads / 128) * kRegsEntry,
               "setmaxnreg budget exceeds the register pool the CTA is launched with (softmax warps would block)");
