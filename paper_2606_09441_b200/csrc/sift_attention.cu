@@ -51,10 +51,13 @@ constexpr int kExpEmuMask = SIFT_EXP_EMU_MASK;   // bit j: pairs with (index & 3
 constexpr int kRegsEntry = (kNQ == 2) ? 128 : 168;               // what __launch_bounds__(kNumThreads, 1) yields
 // 4 warps per sub-partition share 512 registers per lane: 2 x 216 + 2 x 40 (measured: 208/48 -1%, 200/56 -5%, 192/64 -30%:
 // the softmax loop holds a whole 128-column row of S)
-constexpr int kRegsOther = 40;                                   // non-softmax warps after setmaxnreg.dec
+constexpr int kRegsOther = 40;                                   // producer warps after setmaxnreg.dec
+constexpr int kItemWarp = kFirstVWarp + 1;                       // warp 13: item fetch + Q loads; shares sub-partition 1 with
+constexpr int kRegsItem = 24, kRegsMma = 56;                     // the MMA issuer (warp 1), whose loop spilled at 40 registers
 constexpr int kRegsSoftmax = 216;              // softmax warps after setmaxnreg.inc
 
-static_assert(kNQ * kRegsSoftmax + 2 * kRegsOther <= (kNumThreads / 128) * kRegsEntry,
+static_assert(kNQ * kRegsSoftmax + 2 * kRegsOther <= (kNumThreads / 128) * kRegsEntry &&
+              kNQ * kRegsSoftmax + kRegsItem + kRegsMma <= (kNumThreads / 128) * kRegsEntry,
               "setmaxnreg budget exceeds the register pool the CTA is launched with (softmax warps would block)");
 
 #ifdef SIFT_NO_CFENCE
@@ -240,9 +243,9 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 
   // register budget: the four non-softmax warps give registers to the softmax warpgroups (setmaxnreg at the top of
   // every role branch so that it dominates the role's code)
-  if (warp == 0) {
+  if (warp == kItemWarp) {
     // ======================================= item fetch + Q producer =======================================
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsItem));
     const uint32_t q_smem = sbase + S::kQOff;
     for (int it_n = 0;; ++it_n) {
       const int slot = it_n & 1;
@@ -282,7 +285,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       }
       __syncwarp();
     }
-  } else if (warp == 2 || warp == 3 || warp >= kFirstVWarp) {
+  } else if (warp == 0 || warp == 2 || warp == 3 || (warp >= kFirstVWarp && warp != kItemWarp)) {
     // ======================================= K (warps 2,3) / V (last two warps) producers =======================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
     // 64 threads per operand.  Tiled steps (local tiles, dense rows): one thread issues one TMA box per 64-column half.
@@ -292,8 +295,9 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     // gather_mode 1 (SIFT_GATHER_MODE=1) = every thread copies 16-byte pieces of the listed rows with cp.async,
     // applying the 128-byte swizzle by hand (chunk ^= row & 7) so that the landed image is what a tiled box would
     // have written; completion is signalled by cp.async.mbarrier.arrive.  Both are parity-tested.
-    const bool is_k = warp < 4 || warp == kFirstVWarp + 2;
-    const int pw = (warp == kFirstVWarp + 2 || warp == kFirstVWarp + 3) ? 2 : (is_k ? warp - 2 : warp - kFirstVWarp);   // 0..2
+    // K: warps 2, 3, 14; V: warps 0, 12, 15 (sub-partition 1 keeps the MMA issuer and the light item warp: registers)
+    const bool is_k = warp == 2 || warp == 3 || warp == kFirstVWarp + 2;
+    const int pw = is_k ? (warp == 2 ? 0 : (warp == 3 ? 1 : 2)) : (warp == 0 ? 0 : (warp == kFirstVWarp ? 1 : 2));   // 0..2
     const int ptid = pw * 32 + lane;
     const int n_stages = is_k ? S::kKStages : S::kVStages;
     const int b_full = is_k ? S::bKFull : S::bVFull, b_empty = is_k ? S::bKEmpty : S::bVEmpty;
@@ -419,7 +423,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     // memory are re-broadcast with shfl so that ptxas keeps them in uniform registers); one elected lane issues.
     // With a divergent `if (lane == 0)` around the loop every tcgen05.mma operand took an R2UR round trip and the
     // issuing thread itself became the bottleneck (profiles/r1_mma_issue.md).
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsMma));
     uint32_t kst = 0, kph = 0, vst = 0, vph = 0, pph[kNQ];
 #pragma unroll
     for (int q = 0; q < kNQ; ++q) pph[q] = 0;
@@ -693,7 +697,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     }
     }
   } else {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));   // idle warps only donate registers
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));   // (no such warp today: all 16 have a role)
   }
 
   tc_fence_before();

@@ -49,7 +49,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int tag
   uint32_t spins = 0;
   while (!mbar_try_wait(bar, parity)) {
     if (++spins > (1u << 24)) {
+#ifdef SIFT_DEBUG_BARRIERS   // the message costs a printf frame at every wait site (registers, code size): debug builds only
       printf("sift: mbarrier timeout tag=%d block=%d thread=%d parity=%u\n", tag, (int)blockIdx.x, (int)threadIdx.x, parity);
+#endif
       __trap();
     }
   }
