@@ -485,12 +485,22 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     __syncwarp();                                                                                                \
   }
       int pending = 0, fresh = (1 << kNQ) - 1;   // fresh bit q: the next P V of tile q overwrites O instead of accumulating
+      // One loop body serves the steps and the drain iteration after the last step (P V of the last step only, no K
+      // stage): a separate tail would duplicate all the P V issue code (the issuer's loop is ~10 KB of SASS as it is, and
+      // the hot loops of the roles compete for a 32 KB instruction cache).
       bool last = false;
-      for (int j = 0; !last; ++j) {
-        mbar_wait(bar(S::bKFull + kst), kph, 204);
-        const int inf = info[4 + kst];
-        const int act = inf & 3;
-        last = (inf & 4) != 0;
+      for (int j = 0;; ++j) {
+        const bool drain = last;                 // the previous iteration was the item's last step
+        int act = 0;
+        if (!drain) {
+          mbar_wait(bar(S::bKFull + kst), kph, 204);
+          const int inf = info[4 + kst];
+          act = inf & 3;
+          last = (inf & 4) != 0;
+        } else {
+          if (elect_one()) umma_commit(bar(S::bQEmpty));   // every Q K^T of this item has been issued
+          __syncwarp();
+        }
         const uint32_t kt = k_smem + kst * S::kTileBytes, vt = v_smem + vst * S::kTileBytes;
         if (j > 0) mbar_wait(bar(S::bVFull + vst), vph, 203);
         CFENCE();   // cp.async-gathered tiles were written through the generic proxy
@@ -499,25 +509,13 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         if constexpr (kNQ == 2) { SIFT_QK_STEP(1) }
         if (elect_one()) {
           if (j > 0) umma_commit(bar(S::bVEmpty + vst));
-          umma_commit(bar(S::bKEmpty + kst));
+          if (!drain) umma_commit(bar(S::bKEmpty + kst));
         }
         __syncwarp();
         if (j > 0) { if (++vst == S::kVStages) { vst = 0; vph ^= 1; } }
+        if (drain) break;
         if (++kst == S::kKStages) { kst = 0; kph ^= 1; }
         pending = act;
-      }
-      if (elect_one()) umma_commit(bar(S::bQEmpty));   // every Q K^T of this item has been issued
-      __syncwarp();
-      {
-        const uint32_t vt = v_smem + vst * S::kTileBytes;
-        mbar_wait(bar(S::bVFull + vst), vph, 203);
-        CFENCE();
-        tc_fence_after();
-        SIFT_PV_STEP(0)
-        if constexpr (kNQ == 2) { SIFT_PV_STEP(1) }
-        if (elect_one()) umma_commit(bar(S::bVEmpty + vst));
-        __syncwarp();
-        if (++vst == S::kVStages) { vst = 0; vph ^= 1; }
       }
 #undef SIFT_QK_STEP
 #undef SIFT_PV_STEP
