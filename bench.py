@@ -193,7 +193,7 @@ def time_each(fn, steps):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one sparse sift_attention_kernel<128> launch on C3 32K, from the
 # `ncu --set full` capture summarised in profiles/r1_attention_ncu_full.md (algorithmic bytes: Q+K+V+O+LSE = 0.66 GB)
-NCU_DRAM_BYTES_PER_LAUNCH_C3 = 0.822e9
+NCU_DRAM_BYTES_PER_LAUNCH_C3 = 0.809e9
 
 
 def cpu_oracle_sample(w, layer=0, budget_rows=8192, heads=tuple(range(0, 32, 2)), seed=0):
