@@ -3,16 +3,19 @@
 // Paper design (FlashAttention-3 on H200: TMA + wgmma, the N-block index read from sparse_n_indices[i]) is prior art.
 // This kernel keeps the idea "an index list drives which K/V tile the copy engine fetches" and is otherwise built for
 // Blackwell:
-//   * persistent CTAs (one per SM) pull (q-head, M-block) work items, longest first, through an atomic counter;
-//   * an M-block is kNQ query tiles of 128 TMEM lanes of the same document and head: they share the head's cross
-//     list, so every gathered K/V tile in shared memory feeds kNQ accumulators;
-//   * warp roles: warp 0 = work-item fetch + Q tiles (TMA), warp 1 = tcgen05.mma issuer, warps 2/3 = K/V producers (tiled TMA
-//     boxes for local tiles and dense rows; TMA `tile::gather4` for the row-granular cross keys), warps 4.. = one softmax
-//     warpgroup per query tile (one row per thread, S read with tcgen05.ld, P written back to TMEM as bf16 and used
-//     as the A operand of the P*V MMA, lazy rescale of the TMEM-resident O accumulator);
+//   * persistent CTAs (one per SM, 16 warps) pull (q-head, M-block) work items through an atomic counter in the order the
+//     decode's scheduler fixed (kv-head groups sized to the L2, longest first inside a group);
+//   * an M-block is kNQ = 2 query tiles of 128 TMEM lanes of the same document and head: they share the head's cross
+//     list, so every gathered K/V tile in shared memory feeds two accumulators;
+//   * warp roles: warp 13 = work-item fetch + Q tiles (TMA); warp 1 = tcgen05.mma issuer (warp-uniform operands, one
+//     elected lane issues); warps 2, 3, 14 = K producers, warps 0, 12, 15 = V producers (tiled TMA boxes for local tiles,
+//     pages and dense rows; TMA `tile::gather4`, or cp.async, for the row-granular cross keys); warps 4..11 = one softmax
+//     warpgroup per query tile (one row per thread, S read with tcgen05.ld, P written back to TMEM as bf16 in four key
+//     ranges and used as the A operand of the P*V MMAs, lazy rescale of the TMEM-resident O accumulator);
+//   * registers are re-split with setmaxnreg per sub-partition: softmax 216, MMA issuer 56, producers 40, item warp 24;
 //   * S = Q K^T and O += P V are tcgen05.mma.kind::f16 (bf16 in, fp32 accumulate in TMEM).
 // Work decomposition of one DOC item (document d >= 0, head h):
-//   cross phase  groups of 128 entries of cross_idx[h][0 .. cross_ptr[h][d])        (a6 in DESIGN.md)
+//   cross phase  groups of 128 entries of cross_idx[h][0 .. cross_ptr[h][d]) (G = 1; one listed page per step at G = tile)  (a6)
 //   local phase  union of the tiles' local lists; the diagonal tile is causally masked  (a7)
 // and of a DENSE item (user-query rows, or the dense comparator): key blocks 0,128,.. up to the last row (a8).
 #include <cuda.h>
