@@ -111,8 +111,7 @@ struct Smem {
   static constexpr int kNumBars = bItemEmpty + 2;
   static constexpr int kInfoOff = kBarOff + ((kNumBars * 8 + 15) / 16) * 16;
   // info words: [0] tmem base, [1..2] item ring, [4 .. 4+kKStages) per-K-stage step info
-  static constexpr int kXchgOff = kInfoOff + 64;           // row max / row sum exchange between the two column halves
-  static constexpr int kBytes = kXchgOff + 2 * 2 * 128 * 4;
+  static constexpr int kBytes = kInfoOff + 64;
   static_assert(kBytes <= 227 * 1024, "shared memory budget");
 };
 
