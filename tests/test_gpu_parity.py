@@ -370,3 +370,22 @@ def test_randomised_shapes_and_modes(monkeypatch):
         rows = range(n) if n <= 900 else sorted(set(int(x) for x in rng.integers(0, n, 500)) | {0, n - 1})
         mx, mean, le = gu.attention_errors(w, 0, o, lse, range(min(hq, 4)), rows)
         assert mx <= gu.TOL_MAX and mean <= gu.TOL_MEAN and le <= gu.TOL_LSE, (case, mx, mean, le)
+
+
+def test_lse_is_optional_and_strided_inputs():
+    """lse = NULL is allowed (include/sift.h); Q/K/V/O may be row-strided views of wider buffers (row strides are
+    arguments of the ABI): both must give the same O as the plain call."""
+    w = wl.custom("opt", n_q_heads=4, n_kv_heads=2, head_dim=128, doc_lens=(300, 200), query_len=50, tile=128, seed=47)
+    shape, md, o_ref, lse_ref = gu.run_sift(w)
+    q, k, v = (t.cuda() for t in w.qkv(0))
+    o1, l1 = api.sift_prefill_attention(shape, 0, q, k, v, md, return_lse=False)
+    torch.cuda.synchronize()
+    assert l1 is None and torch.equal(o1, o_ref)
+    n = q.shape[0]
+    qb = torch.zeros((n, 6, 128), dtype=torch.bfloat16, device="cuda"); qb[:, :4] = q
+    kb = torch.zeros((n, 3, 128), dtype=torch.bfloat16, device="cuda"); kb[:, :2] = k
+    vb = torch.zeros((n, 3, 128), dtype=torch.bfloat16, device="cuda"); vb[:, :2] = v
+    ob = torch.full((n, 6, 128), 3.0, dtype=torch.bfloat16, device="cuda")
+    o2, l2 = api.sift_prefill_attention(shape, 0, qb[:, :4], kb[:, :2], vb[:, :2], md, ob[:, :4])
+    torch.cuda.synchronize()
+    assert torch.equal(ob[:, :4], o_ref) and torch.equal(l2, lse_ref) and bool((ob[:, 4:] == 3.0).all())
