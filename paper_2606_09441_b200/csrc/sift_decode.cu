@@ -197,7 +197,10 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
     __syncthreads();
   }
   const int NT = s_tile_base[D + 1];
-  const bool writer = (h == 0 && l == 0);
+  // blockIdx.z splits a (layer, head) into its two independent outputs: z = 0 the cross list, z = 1 the local lists
+  // (and, for the first head, the tile tables).  Halves the latency chain of a CTA (a single layer is latency-bound).
+  const bool do_cross = (blockIdx.z == 0);
+  const bool writer = (h == 0 && l == 0 && !do_cross);
   if (writer) {
     for (int d = tid; d <= D + 1; d += kDecodeThreads) p.tile_base[d] = s_tile_base[d];
     for (int d = tid; d <= D; d += kDecodeThreads) {
@@ -214,9 +217,9 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
   // same two barriers) turns the counts into offsets.
   int32_t* cross_ptr = p.cross_ptr + lh * (D + 1);
   int32_t* cross_idx = p.cross_idx + lh * p.cross_cap;
-  const int total_words = s_wstart[D];
+  const int total_words = do_cross ? s_wstart[D] : 0;
   int running = 0;
-  if (tid == 0) cross_ptr[0] = 0;
+  if (do_cross && tid == 0) cross_ptr[0] = 0;
   int scan_no = 0;   // the two scan buffers alternate over ALL scans of the kernel (no trailing barrier needed)
   for (int base = 0; base < total_words; base += kWPT * kDecodeThreads) {
     uint32_t bits[kWPT];
@@ -280,7 +283,10 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
     running += pass_total;
   }
   // entries in [total, roundup128(total)) must be valid rows: the attention kernel gathers whole groups
-  for (int i = running + tid; i < ((running + 127) & ~127); i += kDecodeThreads) cross_idx[i] = 0;
+  if (do_cross) {
+    for (int i = running + tid; i < ((running + 127) & ~127); i += kDecodeThreads) cross_idx[i] = 0;
+    return;
+  }
 
   // ---- local lists: LA row popcounts, offsets, fill -------------------------------------------------
   int32_t* local_cnt = p.local_cnt + lh * NT;
@@ -420,7 +426,7 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   p.n_mblocks = lay.n_mblocks; p.n_items = lay.n_items; p.gran = s->cross_gran;
   p.kv_per_group = sched_kv_heads_per_group((int64_t)s->doc_offsets[s->n_docs] + s->query_len, s->head_dim, s->n_kv_heads);
   cudaGetLastError();
-  sift_decode_lists_kernel<<<dim3(s->n_q_heads, s->n_layers), kDecodeThreads, 0, st>>>(dt, p);
+  sift_decode_lists_kernel<<<dim3(s->n_q_heads, s->n_layers, 2), kDecodeThreads, 0, st>>>(dt, p);
   sift_schedule_kernel<<<s->n_layers, kSchedThreads, 0, st>>>(p, s->n_docs, s->n_layers);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "decode launch: %s", cudaGetErrorString(e));
