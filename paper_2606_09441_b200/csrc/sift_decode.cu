@@ -16,6 +16,7 @@ namespace sift {
 constexpr int kDecodeThreads = 256;
 constexpr int kWPT = 4;    // CA words per thread and pass (a pass = 32768 key bits)
 constexpr int kTPT = 2;    // tiles per thread and pass
+constexpr int kMaxCrossParts = 4;   // CTAs that may share the cross list of one (layer, head) when the grid is small
 constexpr int kStageEntries = 4096;   // shared-memory staging of one chunk: up to 50% of its 8192 bits set
 constexpr int kSchedThreads = 1024;
 constexpr int kCostBuckets = 4096;
@@ -28,6 +29,7 @@ struct DecodeParams {
   int32_t *mblock_tile0, *sched, *counters;
   int32_t n_q_heads, n_kv_heads, n_tiles, cross_cap, local_cap, n_mblocks, n_items, gran;
   int32_t kv_per_group;   // kv heads whose work items are scheduled together (sched_kv_heads_per_group)
+  int32_t cross_parts;    // CTAs per (layer, head) for the cross list: 4 when the grid would not fill the GPU, else 1
 };
 
 // exclusive scan over the block; returns the exclusive prefix of v and (via total) the block sum
@@ -197,9 +199,10 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
     __syncthreads();
   }
   const int NT = s_tile_base[D + 1];
-  // blockIdx.z splits a (layer, head) into its two independent outputs: z = 0 the cross list, z = 1 the local lists
-  // (and, for the first head, the tile tables).  Halves the latency chain of a CTA (a single layer is latency-bound).
-  const bool do_cross = (blockIdx.z == 0);
+  // blockIdx.z splits a (layer, head): z < kCrossParts = one range of the cross list, z = kCrossParts = the local lists
+  // (and, for the first head, the tile tables).  Shortens the latency chain of a CTA (a single layer is latency-bound).
+  const int kCrossParts = p.cross_parts;
+  const bool do_cross = ((int)blockIdx.z < kCrossParts);
   const bool writer = (h == 0 && l == 0 && !do_cross);
   if (writer) {
     for (int d = tid; d <= D + 1; d += kDecodeThreads) p.tile_base[d] = s_tile_base[d];
@@ -217,36 +220,52 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
   // same two barriers) turns the counts into offsets.
   int32_t* cross_ptr = p.cross_ptr + lh * (D + 1);
   int32_t* cross_idx = p.cross_idx + lh * p.cross_cap;
-  const int total_words = do_cross ? s_wstart[D] : 0;
+  // masked stream-order bits of word v of the head's virtual word sequence, the global coordinate of its bit 0 and
+  // the document it closes (or -1)
+  auto load_word = [&](int v, int& key0, int& closes) -> uint32_t {
+    const int d = upper_seg(s_wstart, D, v);
+    const int wi = v - s_wstart[d];
+    const int len = dt.off[d + 1] - dt.off[d];
+    const int nbits = (len + G - 1) / G;
+    const uintptr_t a = reinterpret_cast<uintptr_t>(p.ca) + (uint64_t)(dt.ca_off[d] + lh * ((nbits + 7) >> 3));
+    const int lead = (int)(a & 3) * 8;
+    const uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(a & ~(uintptr_t)3) + wi);
+    // stream bit s (MSB-first within each byte, bytes ascending) -> bit s of x
+    const uint32_t x = __brev(__byte_perm(w, 0, 0x0123));
+    const int lo = max(0, lead - wi * 32);
+    const int hi = min(32, lead + nbits - wi * 32);
+    uint32_t m = (hi >= 32) ? 0xffffffffu : ((1u << hi) - 1u);
+    m &= ~((lo >= 32) ? 0xffffffffu : ((1u << lo) - 1u));
+    // global coordinate of stream bit 0 of this word: key row (G == 1) or tile id (G == tile; a page is a tile)
+    key0 = (G == 1 ? dt.off[d] : s_tile_base[d]) + wi * 32 - lead;
+    closes = (v + 1 == s_wstart[d + 1]) ? d : -1;
+    return x & m;
+  };
+  // The word sequence of a head is cut into kCrossParts ranges, one CTA each (grid z): a CTA first popcounts the words
+  // before its range (the bit vectors of a head are a few KB: re-reading them costs less than waiting for a prefix
+  // from another CTA), which gives it the list offset of its first entry.
+  const int all_words = s_wstart[D];
+  const int per = (all_words + kCrossParts - 1) / kCrossParts;
+  const int w_lo = do_cross ? min(all_words, (int)blockIdx.z * per) : 0;
+  const int total_words = do_cross ? min(all_words, w_lo + per) : 0;      // end of this CTA's range
   int running = 0;
-  if (do_cross && tid == 0) cross_ptr[0] = 0;
+  if (do_cross) {
+    int before = 0, k0, cl;
+    for (int v = tid; v < w_lo; v += kDecodeThreads) before += __popc(load_word(v, k0, cl));
+    int tot;
+    block_exclusive_scan<kDecodeThreads>(before, s_scan, tot);
+    running = tot;
+    if (blockIdx.z == 0 && tid == 0) cross_ptr[0] = 0;
+  }
   int scan_no = 0;   // the two scan buffers alternate over ALL scans of the kernel (no trailing barrier needed)
-  for (int base = 0; base < total_words; base += kWPT * kDecodeThreads) {
+  for (int base = w_lo; base < total_words; base += kWPT * kDecodeThreads) {
     uint32_t bits[kWPT];
     int key0[kWPT], cnt[kWPT], dd[kWPT];
 #pragma unroll
     for (int k = 0; k < kWPT; ++k) {
       const int v = base + k * kDecodeThreads + tid;
       bits[k] = 0; key0[k] = 0; dd[k] = -1;
-      if (v < total_words) {
-        const int d = upper_seg(s_wstart, D, v);
-        const int wi = v - s_wstart[d];
-        const int len = dt.off[d + 1] - dt.off[d];
-        const int nbits = (len + G - 1) / G;
-        const uintptr_t a = reinterpret_cast<uintptr_t>(p.ca) + (uint64_t)(dt.ca_off[d] + lh * ((nbits + 7) >> 3));
-        const int lead = (int)(a & 3) * 8;
-        const uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(a & ~(uintptr_t)3) + wi);
-        // stream bit s (MSB-first within each byte, bytes ascending) -> bit s of x
-        const uint32_t x = __brev(__byte_perm(w, 0, 0x0123));
-        const int lo = max(0, lead - wi * 32);
-        const int hi = min(32, lead + nbits - wi * 32);
-        uint32_t m = (hi >= 32) ? 0xffffffffu : ((1u << hi) - 1u);
-        m &= ~((lo >= 32) ? 0xffffffffu : ((1u << lo) - 1u));
-        bits[k] = x & m;
-        // global coordinate of stream bit 0 of this word: key row (G == 1) or tile id (G == tile; a page is a tile)
-        key0[k] = (G == 1 ? dt.off[d] : s_tile_base[d]) + wi * 32 - lead;
-        if (v + 1 == s_wstart[d + 1]) dd[k] = d;   // last word of document d
-      }
+      if (v < total_words) bits[k] = load_word(v, key0[k], dd[k]);
     }
 #pragma unroll
     for (int k = 0; k < kWPT; ++k) cnt[k] = __popc(bits[k]);                     // pass 1: count
@@ -284,7 +303,8 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
   }
   // entries in [total, roundup128(total)) must be valid rows: the attention kernel gathers whole groups
   if (do_cross) {
-    for (int i = running + tid; i < ((running + 127) & ~127); i += kDecodeThreads) cross_idx[i] = 0;
+    if (blockIdx.z == kCrossParts - 1)
+      for (int i = running + tid; i < ((running + 127) & ~127); i += kDecodeThreads) cross_idx[i] = 0;
     return;
   }
 
@@ -424,9 +444,12 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   p.mblock_tile0 = at(lay.mblock_tile0); p.sched = at(lay.sched); p.counters = at(lay.counters);
   p.n_q_heads = s->n_q_heads; p.n_kv_heads = s->n_kv_heads; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap; p.local_cap = lay.local_cap;
   p.n_mblocks = lay.n_mblocks; p.n_items = lay.n_items; p.gran = s->cross_gran;
+  // few (layer, head) pairs (one layer of an 8B-class model = 32): the call is latency-bound, cut each head's cross list
+  // into ranges for separate CTAs; many (a whole stack = 1024): one CTA per list is more efficient (no re-counting)
+  p.cross_parts = ((int64_t)s->n_q_heads * s->n_layers * 2 <= 2 * 148) ? kMaxCrossParts : 1;
   p.kv_per_group = sched_kv_heads_per_group((int64_t)s->doc_offsets[s->n_docs] + s->query_len, s->head_dim, s->n_kv_heads);
   cudaGetLastError();
-  sift_decode_lists_kernel<<<dim3(s->n_q_heads, s->n_layers, 2), kDecodeThreads, 0, st>>>(dt, p);
+  sift_decode_lists_kernel<<<dim3(s->n_q_heads, s->n_layers, p.cross_parts + 1), kDecodeThreads, 0, st>>>(dt, p);
   sift_schedule_kernel<<<s->n_layers, kSchedThreads, 0, st>>>(p, s->n_docs, s->n_layers);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "decode launch: %s", cudaGetErrorString(e));
