@@ -389,3 +389,21 @@ def test_lse_is_optional_and_strided_inputs():
     o2, l2 = api.sift_prefill_attention(shape, 0, qb[:, :4], kb[:, :2], vb[:, :2], md, ob[:, :4])
     torch.cuda.synchronize()
     assert torch.equal(ob[:, :4], o_ref) and torch.equal(l2, lse_ref) and bool((ob[:, 4:] == 3.0).all())
+
+
+def test_host_pipeline_layer_of_a_stack():
+    """The pipeline addresses the q-heads of layer `layer` inside a multi-layer [layer][q_head][bytes] blob."""
+    from paper_2606_09441_b200.pipeline import HostLayerPipeline
+    w = wl.custom("pipe-l", n_layers=3, n_q_heads=4, n_kv_heads=2, head_dim=64, doc_lens=(300, 129, 64), query_len=40,
+                  tile=64, p_cross=0.3, seed=53)
+    shape, md = gu.decode_on_gpu(w)
+    q, k, v = w.qkv(2)
+    o_ref, lse_ref = api.sift_prefill_attention(shape, 2, q.cuda(), k.cuda(), v.cuda(), md)
+    torch.cuda.synchronize()
+    qh, kh, vh = (t.pin_memory() for t in (q, k, v))
+    la_h, ca_h = torch.from_numpy(w.la_blob).pin_memory(), torch.from_numpy(w.ca_blob).pin_memory()
+    o_h = torch.empty(q.shape, dtype=q.dtype).pin_memory()
+    pipe = HostLayerPipeline(w.shape)
+    pipe.run(la_h, ca_h, w.la_doc_off, w.ca_doc_off, qh, kh, vh, o_h, layer=2)
+    pipe.wait()
+    assert torch.equal(o_h, o_ref.cpu()) and torch.equal(pipe.lse.cpu(), lse_ref.cpu())
