@@ -114,20 +114,25 @@ def sum_over_ranks(x: float, world: int) -> float:
 class GpuCase:
     """One prompt resident on the device + the calls of one step."""
 
-    def __init__(self, w, layer=0):
+    def __init__(self, w, layer=0, qkv_dev=None, host=True):
+        """qkv_dev: device Q/K/V to reuse (legs that only change the bit vectors); host=False skips the pinned copies."""
         from paper_2606_09441_b200 import api, metrics
         self.api, self.w, self.layer = api, w, layer
         self.shape = api.Shape.from_prompt(w.shape)
-        self.la_h = torch.from_numpy(w.la_blob).pin_memory()
-        self.ca_h = torch.from_numpy(w.ca_blob).pin_memory()
-        q, k, v = w.qkv(layer)
-        self.q_h, self.k_h, self.v_h = q.pin_memory(), k.pin_memory(), v.pin_memory()
+        self.la_h, self.ca_h = torch.from_numpy(w.la_blob), torch.from_numpy(w.ca_blob)
+        if qkv_dev is None:
+            q, k, v = w.qkv(layer)
+            if host:
+                self.q_h, self.k_h, self.v_h = q.pin_memory(), k.pin_memory(), v.pin_memory()
+                self.la_h, self.ca_h = self.la_h.pin_memory(), self.ca_h.pin_memory()
+                self.o_h = torch.empty(q.shape, dtype=q.dtype).pin_memory()
+            self.q, self.k, self.v = q.cuda(), k.cuda(), v.cuda()
+        else:
+            self.q, self.k, self.v = qkv_dev
         self.la, self.ca = self.la_h.cuda(), self.ca_h.cuda()
-        self.q, self.k, self.v = self.q_h.cuda(), self.k_h.cuda(), self.v_h.cuda()
         self.md = torch.empty(api.sift_metadata_size(self.shape), dtype=torch.uint8, device="cuda")
         self.o = torch.empty_like(self.q)
-        self.lse = torch.empty((q.shape[1], q.shape[0]), dtype=torch.float32, device="cuda")
-        self.o_h = torch.empty(self.o.shape, dtype=self.o.dtype).pin_memory()
+        self.lse = torch.empty((self.q.shape[1], self.q.shape[0]), dtype=torch.float32, device="cuda")
         self.pipe = None
         self.decode()
         torch.cuda.synchronize()
@@ -191,9 +196,21 @@ def time_each(fn, steps):
     return [a.elapsed_time(b) for a, b in ev]
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one sparse sift_attention_kernel<128> launch on C3 32K, from the
-# `ncu --set full` capture summarised in profiles/r1_attention_ncu_full.md (algorithmic bytes: Q+K+V+O+LSE = 0.66 GB)
-NCU_DRAM_BYTES_PER_LAUNCH_C3 = 0.809e9
+def ncu_dram_bytes_per_launch(workload_name):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one sparse attention launch, from the tracked export
+    profiles/attention_dram_traffic.csv (written from an `ncu --set full` capture; its `source` column names the
+    summary with the full command).  None when no capture of this workload is tracked."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "attention_dram_traffic.csv")
+    if not os.path.exists(path):
+        return None, None
+    hit = None
+    for row in csv.DictReader(open(path)):
+        if row["workload"] == workload_name:
+            hit = row                                  # the last matching line wins (newest capture)
+    if hit is None:
+        return None, None
+    return float(hit["dram_bytes_read"]) + float(hit["dram_bytes_write"]), hit["source"]
 
 
 def cpu_oracle_sample(w, layer=0, budget_rows=8192, heads=tuple(range(0, 32, 2)), seed=0):
@@ -246,7 +263,7 @@ def run_ours(args):
 
     # per-kernel timings (same stream, after the headline region)
     att = time_each(case.attention, args.steps)
-    dec = time_each(case.decode, args.steps)
+    dec = time_each_flushed(case.decode, args.steps)
     den = time_each(case.dense, max(3, args.steps // 4))
     att_ms, dec_ms, den_ms = float(np.mean(att)), float(np.mean(dec)), float(np.mean(den))
     achieved = case.flops / (att_ms * 1e-3) / 1e12
@@ -265,12 +282,12 @@ def run_ours(args):
     sus_tf = case.flops / (sus_ms * 1e-3) / 1e12
 
     extra = {"sustained_attention_ms": sus_ms, "sustained_tflops": sus_tf,
-             "sustained_frac_of_sustained_peak": sus_tf / peaks["bf16_sustained"],
+             "sustained_frac_of_sustained_peak": sus_tf / peaks["bf16_sustained"], "sustained_frac_of_burst_peak": sus_tf / peaks["bf16"],
              "attention_ms": att_ms, "attention_ms_best": float(np.min(att)), "decode_us": dec_ms * 1e3,
              "dense_causal_ms": den_ms, "dense_tflops": case.dense_flops / (den_ms * 1e-3) / 1e12,
              "speedup_vs_dense": den_ms / att_ms, "marked_density": case.flops / case.dense_flops,
              "decode_GBps": case.decode_bytes / (dec_ms * 1e-3) / 1e9, "decode_bytes": case.decode_bytes,
-             "frac_of_sustained_peak": achieved / peaks["bf16_sustained"], "n_tokens": w.shape.n_tokens}
+             "decode_timing": "mean of %d calls, L2 flushed before each" % args.steps, "n_tokens": w.shape.n_tokens}
     if args.config == "32k" and world == 1:
         # offline metadata generation for one 2000-token document of this prompt and layer: pass 1 =
         # dense causal attention of the document alone (row LSE), pass 2 = sift_encode_document
@@ -287,11 +304,17 @@ def run_ours(args):
             c4.step()
         a4 = float(np.mean(time_each(c4.attention, max(3, args.steps // 2))))
         d4 = float(np.mean(time_each(c4.dense, 3)))
-        k4 = float(np.mean(time_each(c4.decode, max(3, args.steps // 2))))
+        k4 = float(np.mean(time_each_flushed(c4.decode, max(3, args.steps // 2))))
         extra["64k"] = {"n_tokens": c4.w.shape.n_tokens, "attention_ms": a4, "effective_tflops": c4.flops / (a4 * 1e-3) / 1e12,
                         "dense_causal_ms": d4, "dense_tflops": c4.dense_flops / (d4 * 1e-3) / 1e12, "decode_us": k4 * 1e3,
                         "frac_of_peak": c4.flops / (a4 * 1e-3) / 1e12 / peaks["bf16"], "marked_density": c4.flops / c4.dense_flops}
         del c4
+    if args.config == "32k" and world == 1 and not args.no_extra_legs:
+        torch.cuda.empty_cache()
+        extra["density_sweep_32k"] = density_sweep_leg(case, peaks, den_ms, max(3, args.steps // 4))
+        extra["paged_32k"] = dict(paged_leg(case, peaks, max(3, args.steps // 4)), row_granular_attention_ms=att_ms,
+                                  row_granular_effective_tflops=achieved)
+        extra["full_stack"] = full_stack_leg(args.layers, peaks)
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -306,9 +329,9 @@ def run_ours(args):
                 "ms_per_step": e2e_ms},
         "roofline": {"bound": "tensor", "kernel": "sift_attention_kernel<128>", "achieved": achieved, "peak": peaks["bf16"],
                      "unit": "TFLOP/s", "frac": achieved / peaks["bf16"],
-                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH_C3 if args.config == "32k" else None,
-                     "traffic_unit": "bytes per launch (ncu dram read+write; algorithmic Q+K+V+O+LSE = %.3g)" % (
-                         (case.q.numel() * 2 + case.k.numel() * 2) * 2 + case.lse.numel() * 4),
+                     "traffic": ncu_dram_bytes_per_launch(w.name)[0],
+                     "traffic_unit": "bytes per launch (ncu dram read+write from %s; algorithmic Q+K+V+O+LSE = %.3g)" % (
+                         ncu_dram_bytes_per_launch(w.name)[1], (case.q.numel() * 2 + case.k.numel() * 2) * 2 + case.lse.numel() * 4),
                      "peak_source": peaks["src"] + " (burst: kernel timed alone over %d launches)" % args.steps},
         "extra": extra,
     }
@@ -322,24 +345,42 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def run_full_stack(args):
-    """BASELINE.json configs[4]: 32 layers of C3's shape, independent bit vectors per (layer, head, doc), the same 16
+_FLUSH = None
+
+
+def flush_l2():
+    """Write a buffer larger than the 126 MB L2 (the decode is timed with a flushed L2)."""
+    global _FLUSH
+    if _FLUSH is None:
+        _FLUSH = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    _FLUSH.zero_()
+
+
+def time_each_flushed(fn, steps):
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        flush_l2()
+        a.record()
+        fn()
+        b.record()
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in ev]
+
+
+def full_stack_leg(L, peaks, sampler=None):
+    """BASELINE.json configs[4]: L layers of C3's shape, independent bit vectors per (layer, head, doc), the same 16
     documents in 4 orderings (vectors and K/V/Q blocks travel with their document); per ordering ONE decode call for all
-    layers + one attention call per layer, timed end to end on the device.  A step = one ordering."""
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
-    torch.cuda.set_device(0)
+    layers + one attention call per layer, timed end to end on the device.  Q/K/V of every layer are resident and drawn
+    by the device generator (workload.qkv_on_device: same recipe, timing only; the parity tests of C5 use the host
+    generator)."""
     from paper_2606_09441_b200 import api, metrics
-    peaks = load_peaks()
-    L = args.layers
     w0 = wl.config_full_stack(wl.BASE_SEED, L)
     orders = wl.stack_orderings(w0, 4)
     la, ca = torch.from_numpy(w0.la_blob).cuda(), torch.from_numpy(w0.ca_blob).cuda()
-    # Q/K/V of the identity ordering, every layer resident (L x 396 MB); re-ordered prompts are row-block permutations
-    qkv = []
-    for layer in range(L):
-        qkv.append(tuple(t.cuda() for t in w0.qkv(layer)))
+    qkv = [w0.qkv_on_device(layer) for layer in range(L)]
     off0 = [int(x) for x in w0.shape.doc_offsets]
     cases = []
+    dec_bytes = 0
     for perm in orders:
         w = w0.reorder(perm)
         shape = api.Shape.from_prompt(w.shape)
@@ -350,6 +391,9 @@ def run_full_stack(args):
         torch.cuda.synchronize()
         views = {k_: t.cpu().numpy() for k_, t in api.metadata_views(shape, md).items()}
         pairs = sum(int(metrics.marked_pairs_per_head(views, layer, w.shape.n_docs).sum()) for layer in range(L))
+        if not cases:
+            dec_bytes = metrics.decode_algorithmic_bytes(w.shape, api.sift_metadata_layout(shape), views)
+        del views
         cases.append((w, shape, rows, md, pairs))
     o = torch.empty_like(qkv[0][0])
     lse = torch.empty((w0.shape.n_q_heads, w0.shape.n_tokens), dtype=torch.float32, device="cuda")
@@ -366,31 +410,80 @@ def run_full_stack(args):
             q, k, v = cur[layer]
             api.sift_prefill_attention(shape, layer, q, k, v, md, o, lse)
 
-    sampler = ClockSampler(0)
     launches0 = api.sift_launch_count()
     total_ms, total_flops = 0.0, 0
-    sampler.start()
+    if sampler is not None:
+        sampler.start()
     for case in cases:
         permute(case[2])
         ordering_step(case)                    # warm-up of this ordering
         torch.cuda.synchronize()
         total_ms += time_region(lambda: ordering_step(case), 1)
         total_flops += metrics.attention_flops(case[4], w0.shape.head_dim)
-    clocks = sampler.stop()
+    clocks = sampler.stop() if sampler is not None else None
     launches = (api.sift_launch_count() - launches0) // 2     # half of them were warm-up
+    w, shape, rows, md, _ = cases[0]
+    dec = time_each_flushed(lambda: api.sift_decode_metadata(shape, la, w.la_doc_off, ca, w.ca_doc_off, md), 10)
+    dec_ms = float(np.median(dec))
     value = total_flops / (total_ms * 1e-3) / 1e12
+    return {"layers": L, "orderings": 4, "ms_per_ordering": total_ms / 4, "ms_per_layer": total_ms / 4 / L,
+            "effective_tflops": value, "frac_of_sustained_peak": value / peaks["bf16_sustained"],
+            "total_tflop": total_flops / 1e12, "gpu_launches": int(launches), "clocks": clocks,
+            "decode_all_layers_us": dec_ms * 1e3, "decode_bytes": dec_bytes,
+            "decode_GBps": dec_bytes / (dec_ms * 1e-3) / 1e9, "decode_frac_of_hbm": dec_bytes / (dec_ms * 1e-3) / 1e9 / peaks["hbm"],
+            "decode_timing": "median of 10, L2 flushed before each call",
+            "data": "Q/K/V drawn on the device (workload.qkv_on_device), %d layers resident" % L,
+            "recipe": w0.recipe, "n_tokens": w0.shape.n_tokens}
+
+
+def run_full_stack(args):
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(0)
+    peaks = load_peaks()
+    r = full_stack_leg(args.layers, peaks, ClockSampler(0))
     print(json.dumps({
-        "metric": METRIC.replace("1 layer", f"{L} layers x 4 orderings"), "value": value, "unit": UNIT, "n_gpus": 1,
-        "steps": 4, "warmup": 4, "ms_per_step": total_ms / 4, "higher_is_better": True, "scaling": "weak",
+        "metric": METRIC.replace("1 layer", f"{args.layers} layers x 4 orderings"), "value": r["effective_tflops"], "unit": UNIT,
+        "n_gpus": 1, "steps": 4, "warmup": 4, "ms_per_step": r["ms_per_ordering"], "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "bf16", "data": "synthetic", "impl": "ours",
-        "config": {"workload": f"BASELINE.json configs[4] full stack: {L} layers of {w0.recipe}; 4 orderings; "
+        "config": {"workload": f"BASELINE.json configs[4] full stack: {args.layers} layers of {r['recipe']}; 4 orderings; "
                                "1 decode call (all layers) + 1 attention call per layer per ordering",
-                   "n_tokens": w0.shape.n_tokens, "l2": "inputs larger than L2, no flush"},
-        "clocks": clocks, "gpu_launches": int(launches),
-        "roofline": {"bound": "tensor", "kernel": "sift_attention_kernel<128>", "achieved": value, "peak": peaks["bf16_sustained"],
-                     "unit": UNIT, "frac": value / peaks["bf16_sustained"], "traffic": None,
-                     "peak_source": peaks["src"] + " (sustained: %.0f ms of back-to-back launches per ordering)" % (total_ms / 4)},
-        "extra": {"ms_per_ordering": total_ms / 4, "ms_per_layer": total_ms / 4 / L, "total_tflop": total_flops / 1e12}}))
+                   "n_tokens": r["n_tokens"], "l2": "inputs larger than L2, no flush"},
+        "clocks": r["clocks"], "gpu_launches": r["gpu_launches"],
+        "roofline": {"bound": "tensor", "kernel": "sift_attention_kernel<128>", "achieved": r["effective_tflops"],
+                     "peak": peaks["bf16_sustained"], "unit": UNIT, "frac": r["frac_of_sustained_peak"], "traffic": None,
+                     "peak_source": peaks["src"] + " (sustained: %.0f ms of back-to-back launches per ordering)" % r["ms_per_ordering"]},
+        "extra": r}))
+
+
+def density_sweep_leg(base_case, peaks, dense_ms, steps):
+    """north_star: "sparse attention time scaling with marked density" (sec 7.2).  C3's prompt and Q/K/V
+    with p_loc = p_cross = p for every head; ms and effective TFLOP/s per point, and ms / (density x dense ms): 1.0 =
+    time exactly proportional to the marked pairs of the dense kernel of the same build."""
+    out = []
+    for p in (0.05, 0.1, 0.2, 0.4, 0.8, 1.0):
+        w = wl.build_workload(f"C3-sweep-p{p}", base_case.w.shape, wl.BASE_SEED + 17, p, p if p < 1.0 else 1.1,
+                              recipe=f"C3 prompt, p_loc = p_cross = {p}")
+        c = GpuCase(w, qkv_dev=(base_case.q, base_case.k, base_case.v), host=False)
+        for _ in range(2):
+            c.attention()
+        ms = float(np.mean(time_each(c.attention, steps)))
+        dens = c.flops / c.dense_flops
+        out.append({"p": p, "marked_density": dens, "attention_ms": ms, "effective_tflops": c.flops / (ms * 1e-3) / 1e12,
+                    "frac_of_peak": c.flops / (ms * 1e-3) / 1e12 / peaks["bf16"], "ms_over_density_x_dense_ms": ms / (dens * dense_ms)})
+        del c
+    return out
+
+
+def paged_leg(base_case, peaks, steps):
+    """page-granular CA (G = T: tiled TMA boxes) against row-granular CA (G = 1: TMA
+    gather4) on C3's prompt and Q/K/V at (nearly) equal marked pairs: the same per-bit densities per head."""
+    w = wl.CONFIGS["32k-paged"]()
+    c = GpuCase(w, qkv_dev=(base_case.q, base_case.k, base_case.v), host=False)
+    for _ in range(2):
+        c.attention()
+    ms = float(np.mean(time_each(c.attention, steps)))
+    return {"paged_attention_ms": ms, "paged_effective_tflops": c.flops / (ms * 1e-3) / 1e12, "paged_marked_density": c.flops / c.dense_flops,
+            "paged_frac_of_peak": c.flops / (ms * 1e-3) / 1e12 / peaks["bf16"]}
 
 
 def run_reference(args):
@@ -426,6 +519,7 @@ def main():
     ap.add_argument("--with-64k", dest="with_64k", action="store_true", default=True)
     ap.add_argument("--no-64k", dest="with_64k", action="store_false")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra-legs", action="store_true", help="skip the density sweep, paged and full-stack legs")
     ap.add_argument("--layers", type=int, default=32, help="layers of --config full-stack")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -96,8 +96,6 @@ int sift_decode_metadata(const sift_shape* shape,
  * row strides in elements (head stride = head_dim); bases and row strides 16-byte aligned.
  * O [N][n_q_heads][head_dim] bf16 dev (out); lse [n_q_heads][N] fp32 dev (out, may be NULL): natural-log
  * log-sum-exp of the scaled logits.  A row with no allowed key gets O = 0, lse = -inf.
- * Environment (read at every call): SIFT_GATHER_MODE=1 gathers the row-granular cross keys with cp.async instead of
- * TMA tile::gather4 (same results; kept for comparison).
  * softmax_scale <= 0 selects 1/sqrt(head_dim).  fp32 accumulation; P is rounded to bf16 before P*V.
  * Calls that use the same (metadata, layer) must be stream-ordered (they share a work counter). */
 int sift_prefill_attention(const sift_shape* shape, int32_t layer,
@@ -106,11 +104,44 @@ int sift_prefill_attention(const sift_shape* shape, int32_t layer,
                            const void* metadata /*dev, from sift_decode_metadata*/,
                            void* O, int64_t o_row_stride, float* lse, float softmax_scale, void* stream);
 
-/* Dense causal attention over n_tokens rows with the same kernel body (no metadata). */
+/* Dense causal attention over n_tokens rows with the same kernel body (no metadata).  Calls may be in flight on
+ * different streams at the same time: each call draws its own work counter (cleared on `stream` before the launch). */
 int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
                                 const void* Q, const void* K, const void* V,
                                 int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
                                 void* O, int64_t o_row_stride, float* lse, float softmax_scale, void* stream);
+
+/* ---- one prefill layer from HOST buffers (sec 4.4: the bit vectors arrive from CPU DRAM with the
+ * retrieved documents; L331 sec 7.4: one H2D copy of the vectors) ----
+ * sift_prefill_layer_host takes the bit-vector blobs, Q, K, V from HOST memory and leaves O (and optionally the row
+ * log-sum-exp) in HOST memory.  The layer is processed per kv-head group (a kv head with its q-heads is an independent
+ * unit of the path): the H2D copy of a group's Q columns, its metadata decode + attention, and the D2H copy of its O
+ * columns run on three internal streams, so both PCIe directions overlap the kernels and each other.  The results
+ * are bit-identical to sift_decode_metadata + sift_prefill_attention over all heads at once.
+ *   ctx        from sift_host_ctx_create on the current device: 3 non-blocking streams + events, NO device memory;
+ *              one call at a time per ctx; destroy with sift_host_ctx_destroy (after the work has completed).
+ *   la_host / ca_host  HOST blobs ([layer][q_head][bytes] per document, all n_layers present) of la_blob_bytes /
+ *              ca_blob_bytes bytes; la_doc_off / ca_doc_off HOST, as in sift_decode_metadata.
+ *   Q_host [N][n_q_heads][head_dim], K_host, V_host [N][n_kv_heads][head_dim], O_host [N][n_q_heads][head_dim] bf16
+ *              HOST (pinned memory for the copies to be asynchronous), row strides in elements; lse_host
+ *              [n_q_heads][N] fp32 HOST or NULL.
+ *   workspace  dev, 256-byte aligned, >= sift_prefill_layer_host_workspace_size() bytes (device copies of the inputs,
+ *              O, LSE and one metadata buffer per kv-head group); owned by the caller.
+ * Ordering: all work is ordered after the work already enqueued on `stream`, and `stream` waits for all of it: after
+ * cudaStreamSynchronize(stream) O_host is complete.  The call itself never synchronises.  Host buffers must stay
+ * valid and unmodified until then.  Errors as everywhere (nothing useful is enqueued after a failure). */
+typedef struct sift_host_ctx sift_host_ctx;
+int sift_host_ctx_create(sift_host_ctx** out);
+int sift_host_ctx_destroy(sift_host_ctx* ctx);
+int sift_prefill_layer_host_workspace_size(const sift_shape* shape, size_t la_blob_bytes, size_t ca_blob_bytes,
+                                           size_t* bytes);
+int sift_prefill_layer_host(sift_host_ctx* ctx, const sift_shape* shape, int32_t layer,
+                            const uint8_t* la_host, size_t la_blob_bytes, const int64_t* la_doc_off /*HOST*/,
+                            const uint8_t* ca_host, size_t ca_blob_bytes, const int64_t* ca_doc_off /*HOST*/,
+                            const void* Q_host, const void* K_host, const void* V_host,
+                            int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
+                            void* O_host, int64_t o_row_stride, float* lse_host /*nullable*/, float softmax_scale,
+                            void* workspace /*dev*/, size_t workspace_bytes, void* stream);
 
 /* ---- offline metadata generation (sec 4.1, L209 sec 4.2, L223 sec 4.4) ----
  * Produces the LA / CA bit vectors of ONE document for the q-heads of one layer from the document's standalone dense
@@ -126,6 +157,8 @@ int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, int32_t n_k
  * bits 0: the [q_head][bytes] slice of a document's blob for one layer.  workspace: dev, 16-byte aligned,
  * >= sift_encode_workspace_size() bytes (per-key counters and per-tile flags; cleared by the call). */
 int sift_encode_workspace_size(int32_t doc_len, int32_t n_q_heads, int32_t tile, size_t* bytes);
+/* bytes of ONE q-head's LA / CA vector of a document: ceil(P(P+1)/16), ceil(ceil(doc_len/cross_gran)/8) */
+int sift_encode_output_sizes(int32_t doc_len, int32_t tile, int32_t cross_gran, size_t* la_bytes, size_t* ca_bytes);
 int sift_encode_document(int32_t doc_len, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, int32_t tile,
                          int32_t cross_gran, const void* Q, const void* K, int64_t q_row_stride, int64_t k_row_stride,
                          const float* lse, float alpha, float beta, float gamma, float softmax_scale,

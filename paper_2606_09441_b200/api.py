@@ -15,7 +15,9 @@ from .build import LIB
 SIFT_OK = 0
 EXPORTS = ("sift_version", "sift_last_error", "sift_metadata_size", "sift_metadata_layout",
            "sift_decode_metadata", "sift_prefill_attention", "sift_dense_causal_attention", "sift_launch_count",
-           "sift_encode_workspace_size", "sift_encode_document")
+           "sift_encode_workspace_size", "sift_encode_output_sizes", "sift_encode_document",
+           "sift_host_ctx_create", "sift_host_ctx_destroy", "sift_prefill_layer_host_workspace_size",
+           "sift_prefill_layer_host")
 
 
 class SiftShape(C.Structure):
@@ -64,6 +66,15 @@ def lib() -> C.CDLL:
         L.sift_encode_document.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p,
                                            C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_float, C.c_float, C.c_float,
                                            C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.sift_encode_output_sizes.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+        L.sift_host_ctx_create.argtypes = [C.POINTER(C.c_void_p)]
+        L.sift_host_ctx_destroy.argtypes = [C.c_void_p]
+        L.sift_prefill_layer_host_workspace_size.argtypes = [C.POINTER(SiftShape), C.c_size_t, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.sift_prefill_layer_host.argtypes = [C.c_void_p, C.POINTER(SiftShape), C.c_int32,
+                                              C.c_void_p, C.c_size_t, C.POINTER(C.c_int64),
+                                              C.c_void_p, C.c_size_t, C.POINTER(C.c_int64),
+                                              C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64,
+                                              C.c_void_p, C.c_int64, C.c_void_p, C.c_float, C.c_void_p, C.c_size_t, C.c_void_p]
         _lib = L
     return _lib
 
@@ -216,9 +227,9 @@ def sift_encode_document(q: torch.Tensor, k: torch.Tensor, lse: torch.Tensor, ti
     assert q.stride(1) == q.shape[2] and k.stride(1) == k.shape[2]
     n, hq, d = q.shape
     hkv = k.shape[1]
-    pt = -(-n // tile)
-    la_bytes, ca_bytes = -(-(pt * (pt + 1) // 2) // 8), -(-(-(-n // cross_gran)) // 8)
-    nb = C.c_size_t()
+    lb, cb, nb = C.c_size_t(), C.c_size_t(), C.c_size_t()
+    _check(lib().sift_encode_output_sizes(n, tile, cross_gran, C.byref(lb), C.byref(cb)), "sift_encode_output_sizes")
+    la_bytes, ca_bytes = int(lb.value), int(cb.value)
     _check(lib().sift_encode_workspace_size(n, hq, tile, C.byref(nb)), "sift_encode_workspace_size")
     ws = torch.empty(nb.value, dtype=torch.uint8, device=q.device)
     la = torch.empty((hq, la_bytes), dtype=torch.uint8, device=q.device)
@@ -227,3 +238,51 @@ def sift_encode_document(q: torch.Tensor, k: torch.Tensor, lse: torch.Tensor, ti
                                       lse.data_ptr(), alpha, beta, gamma, softmax_scale, la.data_ptr(), ca.data_ptr(),
                                       ws.data_ptr(), nb.value, _stream(stream)), "sift_encode_document")
     return la, ca
+
+
+class HostContext:
+    """sift_host_ctx (include/sift.h): the three internal streams + events of sift_prefill_layer_host."""
+
+    def __init__(self):
+        self._h = C.c_void_p()
+        _check(lib().sift_host_ctx_create(C.byref(self._h)), "sift_host_ctx_create")
+
+    def close(self):
+        if self._h:
+            lib().sift_host_ctx_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def sift_prefill_layer_host_workspace_size(shape: Shape, la_blob_bytes: int, ca_blob_bytes: int) -> int:
+    n = C.c_size_t(0)
+    _check(lib().sift_prefill_layer_host_workspace_size(C.byref(shape.c), la_blob_bytes, ca_blob_bytes, C.byref(n)),
+           "sift_prefill_layer_host_workspace_size")
+    return int(n.value)
+
+
+def sift_prefill_layer_host(ctx: HostContext, shape: Shape, layer: int, la_h: torch.Tensor, la_doc_off,
+                            ca_h: torch.Tensor, ca_doc_off, q_h: torch.Tensor, k_h: torch.Tensor, v_h: torch.Tensor,
+                            o_h: torch.Tensor, workspace: torch.Tensor, lse_h: Optional[torch.Tensor] = None,
+                            softmax_scale: float = 0.0, stream=None) -> None:
+    """All *_h tensors are HOST tensors (pinned for asynchronous copies); workspace is a uint8 CUDA tensor of at least
+    sift_prefill_layer_host_workspace_size bytes.  Enqueues only: synchronise `stream` before reading o_h."""
+    for t in (la_h, ca_h, q_h, k_h, v_h, o_h):
+        assert not t.is_cuda
+    assert workspace.is_cuda and workspace.dtype == torch.uint8
+    for t in (q_h, k_h, v_h, o_h):
+        assert t.dtype == torch.bfloat16 and t.dim() == 3 and t.stride(2) == 1 and t.stride(1) == t.shape[2]
+    lo, co = _i64(la_doc_off), _i64(ca_doc_off)
+    rc = lib().sift_prefill_layer_host(ctx._h, C.byref(shape.c), layer,
+                                       la_h.data_ptr(), la_h.numel(), lo.ctypes.data_as(C.POINTER(C.c_int64)),
+                                       ca_h.data_ptr(), ca_h.numel(), co.ctypes.data_as(C.POINTER(C.c_int64)),
+                                       q_h.data_ptr(), k_h.data_ptr(), v_h.data_ptr(), q_h.stride(0), k_h.stride(0),
+                                       v_h.stride(0), o_h.data_ptr(), o_h.stride(0),
+                                       lse_h.data_ptr() if lse_h is not None else None, float(softmax_scale),
+                                       workspace.data_ptr(), workspace.numel(), _stream(stream))
+    _check(rc, "sift_prefill_layer_host")

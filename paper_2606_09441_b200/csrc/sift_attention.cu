@@ -46,10 +46,6 @@ constexpr int kFirstVWarp = 4 + 4 * kNQ;
 constexpr int kProducerThreads = 96;              // per operand: K = warps 2, 3, 14; V = warps 12, 13, 15
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 with a stale max
 constexpr uint32_t kTmemCols = 512;
-#ifndef SIFT_EXP_EMU_MASK
-#define SIFT_EXP_EMU_MASK 0x0
-#endif
-constexpr int kExpEmuMask = SIFT_EXP_EMU_MASK;   // bit j: pairs with (index & 3) == j compute 2^x by polynomial instead of MUFU.EX2
 
 constexpr int kRegsEntry = (kNQ == 2) ? 128 : 168;               // what __launch_bounds__(kNumThreads, 1) yields
 // 4 warps per sub-partition share 512 registers per lane: 2 x 216 + 2 x 40 (measured: 208/48 -1%, 200/56 -5%, 192/64 -30%:
@@ -63,12 +59,6 @@ static_assert(kNQ * kRegsSoftmax + 2 * kRegsOther <= (kNumThreads / 128) * kRegs
               kNQ * kRegsSoftmax + kRegsItem + kRegsMma <= (kNumThreads / 128) * kRegsEntry,
               "setmaxnreg budget exceeds the register pool the CTA is launched with (softmax warps would block)");
 
-#ifdef SIFT_NO_CFENCE
-#define CFENCE() do {} while (0)
-#else
-#define CFENCE() fence_proxy_async()
-#endif
-
 struct AttnParams {
   // metadata (null in dense mode)
   const int32_t *tile_seg, *tile_row0, *tile_rows, *mblock_tile0;
@@ -78,9 +68,6 @@ struct AttnParams {
   int32_t n_items, n_docs, n_tiles, cross_cap, local_cap, n_mblocks;
   int32_t zero;   // always 0 (see the TMEM address note in the kernel)
   int32_t dense;  // 1: every M-block is a DENSE item over n_tokens rows
-  int32_t gather_mode;      // 0: TMA tile::gather4 (default), 1: swizzled cp.async row gather
-  const char *k_ptr, *v_ptr;
-  int64_t k_row_bytes, v_row_bytes;
   int32_t n_tokens, n_q_heads, n_kv_heads, tile;
   int32_t kv_per_group;     // dense comparator: kv heads scheduled together (sched_kv_heads_per_group)
   int32_t paged;            // cross_gran == tile: cross entries are global tile ids, one tiled step each
@@ -290,13 +277,10 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   } else if (warp == 0 || warp == 2 || warp == 3 || (warp >= kFirstVWarp && warp != kItemWarp)) {
     // ======================================= K (warps 2,3) / V (last two warps) producers =======================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
-    // 64 threads per operand.  Tiled steps (local tiles, dense rows): one thread issues one TMA box per 64-column half.
-    // Gathered steps (cross keys, row-granular): gather_mode 0 (default) = TMA `tile::gather4`, one instruction per
-    // lane and 64-column half (ptxas serialises the 32 lanes of a gather4 into a loop of uniform-datapath issues,
-    // ~70 clk each from one warp, which is why two warps per operand issue them: profiles/r1_gather_modes.md).
-    // gather_mode 1 (SIFT_GATHER_MODE=1) = every thread copies 16-byte pieces of the listed rows with cp.async,
-    // applying the 128-byte swizzle by hand (chunk ^= row & 7) so that the landed image is what a tiled box would
-    // have written; completion is signalled by cp.async.mbarrier.arrive.  Both are parity-tested.
+    // 96 threads per operand.  Tiled steps (local tiles, pages, dense rows): one thread issues one TMA box per 64-column
+    // half.  Gathered steps (row-granular cross keys): TMA `tile::gather4`, one instruction per lane and 64-column half
+    // (ptxas serialises the 32 lanes of a gather4 into a loop of uniform-datapath issues, ~70 clk each from one warp,
+    // which is why three warps per operand issue them: profiles/r1_gather_modes.md).
     // K: warps 2, 3, 14; V: warps 0, 12, 15 (sub-partition 1 keeps the MMA issuer and the light item warp: registers)
     const bool is_k = warp == 2 || warp == 3 || warp == kFirstVWarp + 2;
     const int pw = is_k ? (warp == 2 ? 0 : (warp == 3 ? 1 : 2)) : (warp == 0 ? 0 : (warp == kFirstVWarp ? 1 : 2));   // 0..2
@@ -306,13 +290,6 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     const uint32_t ring = sbase + (is_k ? S::kKOff : S::kVOff);
     const CUtensorMap* tm_tile = is_k ? &tm_k : &tm_v;
     const CUtensorMap* tm_gath = is_k ? &tm_kg : &tm_vg;
-    const int64_t row_bytes = is_k ? p.k_row_bytes : p.v_row_bytes;
-    constexpr int CH = HD / 8;          // 16-byte chunks per row
-    constexpr int RPP = 64 / CH;        // rows per pass of the 64 threads
-    constexpr int PASSES = kBN / RPP;
-    constexpr int PCH = 16;             // passes per batch of index loads
-    const int c = ptid % CH, rr = ptid / CH;
-    const uint32_t dst_thr = (uint32_t)((c >> 3) * (kBN * 128) + rr * 128);
     uint32_t st = 0, ph = 0;
     for (int it_n = 0;; ++it_n) {
       const int slot = it_n & 1;
@@ -322,34 +299,10 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       if (lane == 0) mbar_arrive(bar(S::bItemEmpty + slot));
       if (code < 0) break;
       const Item it = load_item(p, code);
-      const char* col = (is_k ? p.k_ptr : p.v_ptr) + (int64_t)it.kvh * (HD * 2) + c * 16;
       auto emit = [&](bool gather, int src, int act, bool last) {
         // src: gather -> index of the first cross entry of the group; tiled -> first key row
         const uint32_t full = bar(b_full + st), dst = ring + st * S::kTileBytes;
-        if (gather && p.gather_mode == 1 && pw == 2) {
-          mbar_wait(bar(b_empty + st), ph ^ 1, 401);
-          mbar_arrive(full);                     // the third warp only helps with TMA gathers
-        } else if (gather && p.gather_mode == 1) {
-          const int32_t* ip = p.cross_idx + (int64_t)it.h * p.cross_cap + src + rr;
-          int rows[PCH];
-#pragma unroll
-          for (int j = 0; j < PCH; ++j) rows[j] = __ldg(ip + j * RPP);
-          mbar_wait(bar(b_empty + st), ph ^ 1, 401);
-          if (is_k && ptid == 0) info[4 + st] = act | (last ? 4 : 0);
-#pragma unroll
-          for (int p0 = 0; p0 < PASSES; p0 += PCH) {
-#pragma unroll
-            for (int j = 0; j < PCH; ++j) {
-              const int row = (p0 + j) * RPP + rr;
-              cp_async16(dst + dst_thr + (p0 + j) * RPP * 128 + (((c & 7) ^ (row & 7)) << 4), col + (int64_t)rows[j] * row_bytes);
-            }
-            if (p0 + PCH < PASSES) {
-#pragma unroll
-              for (int j = 0; j < PCH; ++j) rows[j] = __ldg(ip + (p0 + PCH + j) * RPP);
-            }
-          }
-          cp_async_mbar_arrive_noinc(full);
-        } else {
+        {
           // gather4 slots: 2 halves x 32 groups of 4 rows = 64 per tile, spread 22 / 22 / 20 over the three warps
           const int g = pw * 22 + lane;
           const bool g_on = gather && lane < 22 && g < 32 * S::kHalves;
@@ -392,11 +345,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           const int32_t* cidx = p.cross_idx + (int64_t)it.h * p.cross_cap;
           for (int e = 0; e < it.cp; ++e) emit(false, p.tile_row0[cidx[e]], present, e == it.cp - 1 && nloc == 0);
         }
-#if defined(SIFT_ABL) && SIFT_ABL == 3   // timing ablation only (wrong results): cross groups loaded as tiled boxes
-        for (int g = 0; g < ngroups; ++g) emit(false, g * kBN, present, g == ngroups - 1 && nloc == 0);
-#else
         for (int g = 0; g < ngroups; ++g) emit(true, g * kBN, present, g == ngroups - 1 && nloc == 0);
-#endif
         const int32_t* lidx = p.local_idx + (int64_t)it.h * p.local_cap;
         int pos[kNQ];
 #pragma unroll
@@ -505,7 +454,6 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         }
         const uint32_t kt = k_smem + kst * S::kTileBytes, vt = v_smem + vst * S::kTileBytes;
         if (j > 0) mbar_wait(bar(S::bVFull + vst), vph, 203);
-        CFENCE();   // cp.async-gathered tiles were written through the generic proxy
         tc_fence_after();
         SIFT_QK_STEP(0)
         if constexpr (kNQ == 2) { SIFT_QK_STEP(1) }
@@ -571,9 +519,6 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         mbar_wait(bar(S::bSFull + q), sph, 301);
         sph ^= 1;
         tc_fence_after();
-#if defined(SIFT_ABL) && SIFT_ABL == 2
-        tc_fence_before(); for (int part = 0; part < kPvParts; ++part) mbar_arrive(bar(S::bPFull + part * kNQ + q)); ++pv_cnt; l = 1.f; m = 0.f; continue;
-#endif
         float s[kBN];
         {
           uint32_t raw0[32], raw1[32], raw2[32], raw3[32];
@@ -629,16 +574,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
             const float2 x = fma2(make_float2(s[c * 32 + 2 * i], s[c * 32 + 2 * i + 1]), sl2, nm2);
-            float2 pr;
-            if ((kExpEmuMask >> (i & 3)) & 1) {
-              pr = ex2_poly2(x);                 // this pair on the FMA pipe: the MUFU is the co-bottleneck (DESIGN 5.2)
-            } else {
-#if defined(SIFT_ABL) && SIFT_ABL == 1
-              pr = x;
-#else
-              pr = make_float2(ex2(x.x), ex2(x.y));
-#endif
-            }
+            const float2 pr = make_float2(ex2(x.x), ex2(x.y));
             if (i & 1) sum_b = add2(sum_b, pr); else sum_a = add2(sum_a, pr);
             pk[i] = pack_bf16x2(pr.x, pr.y);
           }
@@ -709,39 +645,12 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static EncodeTiledFn get_encode_fn() {
-  static EncodeTiledFn fn = nullptr;
-  if (fn) return fn;
-  void* sym = nullptr;
-  cudaDriverEntryPointQueryResult qres;
-  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess ||
-      qres != cudaDriverEntryPointSuccess)
-    return nullptr;
-  fn = reinterpret_cast<EncodeTiledFn>(sym);
-  return fn;
-}
-
-// 2-D bf16 tensor [rows][cols] with row stride `row_stride` elements; box = 64 columns x box_rows, 128B swizzle
-static int make_map(CUtensorMap* m, const void* base, int64_t rows, int64_t cols, int64_t row_stride, int box_rows) {
-  EncodeTiledFn fn = get_encode_fn();
-  if (!fn) return set_error(SIFT_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
-  cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
-  cuuint64_t gstr[1] = {(cuuint64_t)row_stride * 2};
-  cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
-  cuuint32_t estr[2] = {1, 1};
-  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstr, box, estr,
-                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return set_error(SIFT_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
-  return SIFT_OK;
-}
-
-static int g_num_sms = 0;
-__device__ int32_t g_dense_counters[2] = {0, 0};
+// Work counters of the dense comparator: every call takes the next pair of a ring and clears it on its own stream
+// before the launch, so dense calls in flight on different streams never share a counter (the sparse call keeps its
+// counters inside the caller's metadata buffer, one pair per layer).
+constexpr int kDenseCounterRing = 1024;
+__device__ int32_t g_dense_counters[kDenseCounterRing][2];
+static std::atomic<uint32_t> g_dense_ticket{0};
 
 static int check_tensor(const void* ptr, int64_t stride, const char* name) {
   if (!ptr) return set_error(SIFT_ERR_INVALID_ARG, "%s is NULL", name);
@@ -755,28 +664,18 @@ static int launch_attention(AttnParams& p, const void* Q, const void* K, const v
                             cudaStream_t st) {
   CUtensorMap tq, tk, tv, tkg, tvg;
   int rc;
-  p.k_ptr = static_cast<const char*>(K); p.v_ptr = static_cast<const char*>(V);
-  p.k_row_bytes = ks * 2; p.v_row_bytes = vs * 2;
-  { const char* e = getenv("SIFT_GATHER_MODE"); p.gather_mode = (e && e[0] == '1') ? 1 : 0; }  // 1 = cp.async row gather
   const int64_t n = p.n_tokens;
-  if ((rc = make_map(&tq, Q, n, (int64_t)p.n_q_heads * HD, qs, kBM))) return rc;
-  if ((rc = make_map(&tk, K, n, (int64_t)p.n_kv_heads * HD, ks, kBN))) return rc;
-  if ((rc = make_map(&tv, V, n, (int64_t)p.n_kv_heads * HD, vs, kBN))) return rc;
-  if ((rc = make_map(&tkg, K, n, (int64_t)p.n_kv_heads * HD, ks, 1))) return rc;
-  if ((rc = make_map(&tvg, V, n, (int64_t)p.n_kv_heads * HD, vs, 1))) return rc;
-  if (g_num_sms == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-    if (g_num_sms <= 0) g_num_sms = 148;
-  }
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(sift_attention_kernel<HD>, cudaFuncAttributeMaxDynamicSharedMemorySize, Smem<HD>::kBytes);
-    if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "cudaFuncSetAttribute(smem=%d): %s", Smem<HD>::kBytes, cudaGetErrorString(e));
-    attr_set = true;
-  }
-  const int grid = p.n_items < g_num_sms ? (p.n_items > 0 ? p.n_items : 1) : g_num_sms;
+  if ((rc = make_tensor_map_2d(&tq, Q, n, (int64_t)p.n_q_heads * HD, qs, kBM))) return rc;
+  if ((rc = make_tensor_map_2d(&tk, K, n, (int64_t)p.n_kv_heads * HD, ks, kBN))) return rc;
+  if ((rc = make_tensor_map_2d(&tv, V, n, (int64_t)p.n_kv_heads * HD, vs, kBN))) return rc;
+  if ((rc = make_tensor_map_2d(&tkg, K, n, (int64_t)p.n_kv_heads * HD, ks, 1))) return rc;
+  if ((rc = make_tensor_map_2d(&tvg, V, n, (int64_t)p.n_kv_heads * HD, vs, 1))) return rc;
+  int num_sms = 0;
+  if ((rc = device_sm_count(&num_sms))) return rc;
+  if ((rc = ensure_dynamic_smem(reinterpret_cast<const void*>(&sift_attention_kernel<HD>), Smem<HD>::kBytes,
+                                HD == 128 ? kSmemSlotAttn128 : kSmemSlotAttn64)))
+    return rc;
+  const int grid = p.n_items < num_sms ? (p.n_items > 0 ? p.n_items : 1) : num_sms;
   cudaGetLastError();
   sift_attention_kernel<HD><<<grid, kNumThreads, Smem<HD>::kBytes, st>>>(tq, tk, tv, tkg, tvg, p);
   cudaError_t e = cudaGetLastError();
@@ -852,7 +751,9 @@ extern "C" int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, 
   p.n_items = p.n_mblocks * n_q_heads;
   void* cptr = nullptr;
   if (cudaGetSymbolAddress(&cptr, g_dense_counters) != cudaSuccess) return set_error(SIFT_ERR_CUDA, "no device symbol");
-  p.counters = static_cast<int32_t*>(cptr);
+  p.counters = static_cast<int32_t*>(cptr) + 2 * (g_dense_ticket.fetch_add(1, std::memory_order_relaxed) % kDenseCounterRing);
+  if (cudaMemsetAsync(p.counters, 0, 2 * sizeof(int32_t), (cudaStream_t)stream) != cudaSuccess)
+    return set_error(SIFT_ERR_CUDA, "cudaMemsetAsync(dense counters) failed");
   p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
   const float sc = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf((float)head_dim);
   p.scale_log2 = sc * 1.4426950408889634f;

@@ -446,7 +446,9 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   p.n_mblocks = lay.n_mblocks; p.n_items = lay.n_items; p.gran = s->cross_gran;
   // few (layer, head) pairs (one layer of an 8B-class model = 32): the call is latency-bound, cut each head's cross list
   // into ranges for separate CTAs; many (a whole stack = 1024): one CTA per list is more efficient (no re-counting)
-  p.cross_parts = ((int64_t)s->n_q_heads * s->n_layers * 2 <= 2 * 148) ? kMaxCrossParts : 1;
+  int num_sms = 0;
+  if (int rc = device_sm_count(&num_sms)) return rc;
+  p.cross_parts = ((int64_t)s->n_q_heads * s->n_layers <= num_sms) ? kMaxCrossParts : 1;
   p.kv_per_group = sched_kv_heads_per_group((int64_t)s->doc_offsets[s->n_docs] + s->query_len, s->head_dim, s->n_kv_heads);
   cudaGetLastError();
   sift_decode_lists_kernel<<<dim3(s->n_q_heads, s->n_layers, p.cross_parts + 1), kDecodeThreads, 0, st>>>(dt, p);

@@ -205,31 +205,6 @@ sift_encode_pack_kernel(const EncParams p, float gamma, uint8_t* la_out, uint8_t
   }
 }
 
-typedef CUresult (*EncEncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static int enc_make_map(CUtensorMap* m, const void* base, int64_t rows, int64_t cols, int64_t row_stride) {
-  static EncEncodeTiledFn fn = nullptr;
-  if (!fn) {
-    void* sym = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess ||
-        qres != cudaDriverEntryPointSuccess)
-      return set_error(SIFT_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
-    fn = reinterpret_cast<EncEncodeTiledFn>(sym);
-  }
-  cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
-  cuuint64_t gstr[1] = {(cuuint64_t)row_stride * 2};
-  cuuint32_t box[2] = {64, 128};
-  cuuint32_t estr[2] = {1, 1};
-  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstr, box, estr,
-                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return set_error(SIFT_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
-  return SIFT_OK;
-}
-
 static int enc_check(int32_t doc_len, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, int32_t tile, int32_t gran) {
   if (doc_len < 1 || doc_len > (1 << 20) || n_q_heads < 1 || n_q_heads > 255 || n_kv_heads < 1 || n_q_heads % n_kv_heads)
     return set_error(SIFT_ERR_INVALID_ARG, "bad dimensions");
@@ -243,14 +218,11 @@ template <int HD>
 static int enc_launch(const EncParams& p, const void* Q, const void* K, int64_t qs, int64_t ks, cudaStream_t st) {
   CUtensorMap tq, tk;
   int rc;
-  if ((rc = enc_make_map(&tq, Q, p.doc_len, (int64_t)p.n_q_heads * HD, qs))) return rc;
-  if ((rc = enc_make_map(&tk, K, p.doc_len, (int64_t)p.n_kv_heads * HD, ks))) return rc;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(sift_encode_scores_kernel<HD>, cudaFuncAttributeMaxDynamicSharedMemorySize, EncSmem<HD>::kBytes);
-    if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
-    attr_set = true;
-  }
+  if ((rc = make_tensor_map_2d(&tq, Q, p.doc_len, (int64_t)p.n_q_heads * HD, qs, 128))) return rc;
+  if ((rc = make_tensor_map_2d(&tk, K, p.doc_len, (int64_t)p.n_kv_heads * HD, ks, 128))) return rc;
+  if ((rc = ensure_dynamic_smem(reinterpret_cast<const void*>(&sift_encode_scores_kernel<HD>), EncSmem<HD>::kBytes,
+                                HD == 128 ? kSmemSlotEnc128 : kSmemSlotEnc64)))
+    return rc;
   sift_encode_scores_kernel<HD><<<dim3(p.len128 / 128, p.n_q_heads), kEncThreads, EncSmem<HD>::kBytes, st>>>(tq, tk, p);
   return SIFT_OK;
 }
@@ -264,6 +236,16 @@ extern "C" int sift_encode_workspace_size(int32_t doc_len, int32_t n_q_heads, in
   if (doc_len < 1 || n_q_heads < 1 || (tile != 64 && tile != 128)) return set_error(SIFT_ERR_INVALID_ARG, "bad dimensions");
   const int64_t len128 = (doc_len + 127) / 128 * 128, pt = (doc_len + tile - 1) / tile;
   *bytes = (size_t)n_q_heads * (size_t)(len128 + pt * (pt + 1) / 2) * 4;
+  return SIFT_OK;
+}
+
+extern "C" int sift_encode_output_sizes(int32_t doc_len, int32_t tile, int32_t cross_gran, size_t* la_bytes, size_t* ca_bytes) {
+  if (!la_bytes || !ca_bytes) return set_error(SIFT_ERR_INVALID_ARG, "NULL pointer");
+  if (doc_len < 1 || (tile != 64 && tile != 128) || (cross_gran != 1 && cross_gran != tile))
+    return set_error(SIFT_ERR_INVALID_ARG, "bad dimensions");
+  const int64_t pt = (doc_len + tile - 1) / tile, nb = (doc_len + cross_gran - 1) / cross_gran;
+  *la_bytes = (size_t)((pt * (pt + 1) / 2 + 7) / 8);
+  *ca_bytes = (size_t)((nb + 7) / 8);
   return SIFT_OK;
 }
 

@@ -44,6 +44,71 @@ int validate_shape(const sift_shape* s) {
   return SIFT_OK;
 }
 
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int make_tensor_map_2d(CUtensorMap* m, const void* base, int64_t rows, int64_t cols, int64_t row_stride, int box_rows) {
+  static std::atomic<EncodeTiledFn> cached{nullptr};
+  EncodeTiledFn fn = cached.load(std::memory_order_acquire);
+  if (!fn) {
+    void* sym = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+      return set_error(SIFT_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+    fn = reinterpret_cast<EncodeTiledFn>(sym);
+    cached.store(fn, std::memory_order_release);
+  }
+  cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t gstr[1] = {(cuuint64_t)row_stride * 2};
+  cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstr, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return set_error(SIFT_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  return SIFT_OK;
+}
+
+// Per-device launch state: the SM count sizes the persistent grids, the shared-memory opt-in is a per-device
+// attribute of each kernel (a process may call the library on several devices, from several threads).
+constexpr int kMaxDevices = 64;
+struct DeviceState {
+  std::atomic<int> num_sms{0};
+  std::atomic<int> smem_set[kSmemSlots];
+};
+static DeviceState g_dev[kMaxDevices];
+
+static int current_device(int* dev) {
+  if (cudaGetDevice(dev) != cudaSuccess || *dev < 0 || *dev >= kMaxDevices)
+    return set_error(SIFT_ERR_CUDA, "no usable current CUDA device");
+  return SIFT_OK;
+}
+
+int device_sm_count(int* num_sms) {
+  int dev, rc;
+  if ((rc = current_device(&dev))) return rc;
+  int n = g_dev[dev].num_sms.load(std::memory_order_relaxed);
+  if (n == 0) {
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+      return set_error(SIFT_ERR_CUDA, "cannot read the SM count of device %d", dev);
+    g_dev[dev].num_sms.store(n, std::memory_order_relaxed);
+  }
+  *num_sms = n;
+  return SIFT_OK;
+}
+
+int ensure_dynamic_smem(const void* func, int bytes, int slot) {
+  int dev, rc;
+  if ((rc = current_device(&dev))) return rc;
+  if (g_dev[dev].smem_set[slot].load(std::memory_order_acquire)) return SIFT_OK;
+  cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "cudaFuncSetAttribute(smem=%d): %s", bytes, cudaGetErrorString(e));
+  g_dev[dev].smem_set[slot].store(1, std::memory_order_release);
+  return SIFT_OK;
+}
+
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 int compute_layout(const sift_shape* s, sift_md_layout* out) {

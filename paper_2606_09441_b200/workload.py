@@ -148,6 +148,33 @@ class Workload:
             v[a:b] = xv.to(torch.bfloat16)
         return q, k, v
 
+    def qkv_on_device(self, layer: int, device: str = "cuda") -> Tuple[torch.Tensor, torch.Tensor, torch.Tensor]:
+        """Same recipe as ``qkv`` (N(0,1) per (layer, document id), optional per-head scales, rounded to bf16) drawn by
+        the DEVICE generator: a different random stream, so NOT the arrays the oracle sees.  For timing legs that need
+        many layers resident (bench.py full-stack: 32 layers would take minutes on the host generator); every parity
+        test uses ``qkv``."""
+        sh = self.shape
+        n = sh.n_tokens
+        dev = torch.device(device)
+        q = torch.empty((n, sh.n_q_heads, sh.head_dim), dtype=torch.bfloat16, device=dev)
+        k = torch.empty((n, sh.n_kv_heads, sh.head_dim), dtype=torch.bfloat16, device=dev)
+        v = torch.empty((n, sh.n_kv_heads, sh.head_dim), dtype=torch.bfloat16, device=dev)
+        off = sh.doc_offsets
+        segs = [(int(off[p]), int(off[p + 1]), self.doc_ids[p]) for p in range(sh.n_docs)] + [(int(off[-1]), n, 1 << 20)]
+        qs = None if self.q_scale is None else torch.from_numpy(self.q_scale[layer].astype(np.float32)).to(dev)
+        ks = None if self.k_scale is None else torch.from_numpy(self.k_scale[layer].astype(np.float32)).to(dev)
+        g = torch.Generator(device=dev)
+        for (a, b, did) in segs:
+            if b <= a:
+                continue
+            for t, sid, heads, sc in ((q, _S_Q, sh.n_q_heads, qs), (k, _S_K, sh.n_kv_heads, ks), (v, _S_V, sh.n_kv_heads, None)):
+                g.manual_seed(int(_torch_gen(self.seed, sid, layer, did).initial_seed()))
+                x = torch.randn((b - a, heads, sh.head_dim), generator=g, device=dev)
+                if sc is not None:
+                    x = x * sc[None, :, None]
+                t[a:b] = x.to(torch.bfloat16)
+        return q, k, v
+
     # -- re-ordering ------------------------------------------------------------------
     def reorder(self, perm: Sequence[int], name: Optional[str] = None) -> "Workload":
         """Prompt whose position p holds the document that stood at position perm[p]."""

@@ -19,6 +19,11 @@ extern int cudaMemcpy(void* dst, const void* src, size_t n, int kind);
 extern int cudaMemset(void* p, int v, size_t n);
 extern int cudaDeviceSynchronize(void);
 extern int cudaFree(void* p);
+extern int cudaMallocHost(void** p, size_t n);
+extern int cudaFreeHost(void* p);
+extern int cudaStreamCreate(void** s);
+extern int cudaStreamSynchronize(void* s);
+extern int cudaStreamDestroy(void* s);
 
 static uint16_t f2bf(float f) { uint32_t u; memcpy(&u, &f, 4); u += 0x7fffu + ((u >> 16) & 1u); return (uint16_t)(u >> 16); }
 static float bf2f(uint16_t h) { uint32_t u = (uint32_t)h << 16; float f; memcpy(&f, &u, 4); return f; }
@@ -40,6 +45,12 @@ static int host_part(void) {
   CHECK(sift_metadata_size(&s, &nb) == SIFT_ERR_INVALID_ARG);
   CHECK(sift_metadata_size(NULL, &nb) == SIFT_ERR_INVALID_ARG);
   CHECK(sift_encode_workspace_size(300, 4, 128, &nb) == SIFT_OK && nb == 4u * (384u + 6u) * 4u);
+  size_t lb = 0, cb = 0;
+  CHECK(sift_encode_output_sizes(1024, 128, 128, &lb, &cb) == SIFT_OK && lb == 5 && cb == 1);   /* P = 8 -> 36 / 8 bits */
+  CHECK(sift_encode_output_sizes(300, 128, 1, &lb, &cb) == SIFT_OK && lb == 1 && cb == 38);
+  off[2] = 500;
+  CHECK(sift_prefill_layer_host_workspace_size(&s, 100, 100, &nb) == SIFT_OK && nb > 2u * 570u * 4u * 128u * 2u);
+  CHECK(sift_prefill_layer_host(NULL, &s, 0, NULL, 0, NULL, NULL, 0, NULL, NULL, NULL, NULL, 0, 0, 0, NULL, 0, NULL, 0.f, NULL, 0, NULL) == SIFT_ERR_INVALID_ARG);
   printf("abi_smoke host ok\n");
   return 0;
 }
@@ -78,13 +89,16 @@ static int gpu_part(void) {
   CHECK(cudaMalloc(&d_q, qb) == 0 && cudaMalloc(&d_k, kb) == 0 && cudaMalloc(&d_v, kb) == 0 && cudaMalloc(&d_o, qb) == 0 && cudaMalloc(&d_lse, (size_t)HQ * N * 4) == 0);
   CHECK(cudaMemcpy(d_q, hq, qb, 1) == 0 && cudaMemcpy(d_k, hk, kb, 1) == 0 && cudaMemcpy(d_v, hv, kb, 1) == 0);
   uint16_t* ho = (uint16_t*)malloc(qb);
+  uint16_t* ho_sparse = (uint16_t*)malloc(qb);
   float* hl = (float*)malloc((size_t)HQ * N * 4);
+  float* hl_sparse = (float*)malloc((size_t)HQ * N * 4);
   for (int pass = 0; pass < 2; ++pass) {
     CHECK(cudaMemset(d_o, 0xff, qb) == 0);
     int rc = pass == 0 ? sift_prefill_attention(&s, 0, d_q, d_k, d_v, HQ * D, HKV * D, HKV * D, d_md, d_o, HQ * D, (float*)d_lse, 0.f, NULL)
                        : sift_dense_causal_attention(N, HQ, HKV, D, d_q, d_k, d_v, HQ * D, HKV * D, HKV * D, d_o, HQ * D, (float*)d_lse, 0.f, NULL);
     CHECK(rc == SIFT_OK);
     CHECK(cudaDeviceSynchronize() == 0 && cudaMemcpy(ho, d_o, qb, 2) == 0 && cudaMemcpy(hl, d_lse, (size_t)HQ * N * 4, 2) == 0);
+    if (pass == 0) { memcpy(ho_sparse, ho, qb); memcpy(hl_sparse, hl, (size_t)HQ * N * 4); }
     double sum = 0;
     for (int n = 0; n < N; ++n) {
       sum += (double)(n % 64);
@@ -96,6 +110,30 @@ static int gpu_part(void) {
     }
   }
   CHECK(sift_launch_count() >= 4);
+  /* the same layer from HOST buffers through sift_prefill_layer_host: host -> host, bit-identical to the single call */
+  {
+    void *p_la, *p_ca, *p_q, *p_k, *p_v, *p_o, *p_lse, *d_ws, *st;
+    size_t wsb = 0;
+    sift_host_ctx* ctx = NULL;
+    CHECK(cudaMallocHost(&p_la, sizeof(la)) == 0 && cudaMallocHost(&p_ca, sizeof(ca)) == 0 && cudaMallocHost(&p_q, qb) == 0 &&
+          cudaMallocHost(&p_k, kb) == 0 && cudaMallocHost(&p_v, kb) == 0 && cudaMallocHost(&p_o, qb) == 0 &&
+          cudaMallocHost(&p_lse, (size_t)HQ * N * 4) == 0);
+    memcpy(p_la, la, sizeof(la)); memcpy(p_ca, ca, sizeof(ca)); memcpy(p_q, hq, qb); memcpy(p_k, hk, kb); memcpy(p_v, hv, kb);
+    memset(p_o, 0xff, qb);
+    CHECK(sift_prefill_layer_host_workspace_size(&s, sizeof(la), sizeof(ca), &wsb) == SIFT_OK);
+    CHECK(cudaMalloc(&d_ws, wsb) == 0 && cudaStreamCreate(&st) == 0 && sift_host_ctx_create(&ctx) == SIFT_OK);
+    CHECK(sift_prefill_layer_host(ctx, &s, 0, (const uint8_t*)p_la, sizeof(la), la_off, (const uint8_t*)p_ca, sizeof(ca), ca_off,
+                                  p_q, p_k, p_v, HQ * D, HKV * D, HKV * D, p_o, HQ * D, (float*)p_lse, 0.f, d_ws, wsb - 1, st) == SIFT_ERR_WORKSPACE);
+    for (int rep = 0; rep < 2; ++rep) {
+      CHECK(sift_prefill_layer_host(ctx, &s, 0, (const uint8_t*)p_la, sizeof(la), la_off, (const uint8_t*)p_ca, sizeof(ca), ca_off,
+                                    p_q, p_k, p_v, HQ * D, HKV * D, HKV * D, p_o, HQ * D, (float*)p_lse, 0.f, d_ws, wsb, st) == SIFT_OK);
+      CHECK(cudaStreamSynchronize(st) == 0);
+      CHECK(memcmp(p_o, ho_sparse, qb) == 0 && memcmp(p_lse, hl_sparse, (size_t)HQ * N * 4) == 0);
+    }
+    CHECK(sift_host_ctx_destroy(ctx) == SIFT_OK);
+    cudaStreamDestroy(st); cudaFree(d_ws);
+    cudaFreeHost(p_la); cudaFreeHost(p_ca); cudaFreeHost(p_q); cudaFreeHost(p_k); cudaFreeHost(p_v); cudaFreeHost(p_o); cudaFreeHost(p_lse);
+  }
   cudaFree(d_la); cudaFree(d_ca); cudaFree(d_md); cudaFree(d_q); cudaFree(d_k); cudaFree(d_v); cudaFree(d_o); cudaFree(d_lse);
   printf("abi_smoke gpu ok\n");
   return 0;

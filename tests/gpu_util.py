@@ -41,13 +41,51 @@ def assert_metadata_equal(w, shape, md, layers=None):
             assert np.all((pad >= 0) & (pad < w.shape.n_tokens)), "pad entries must be valid rows"
             nl = int(ref["local_ptr"][l, h, -1])
             assert np.array_equal(v["local_idx"][l, h, :nl], ref["local_idx"][l, h, :nl]), ("local_idx", l, h)
-    # scheduler (private): a permutation of all (head, M-block) items
+    # scheduler (private): a permutation of all (head, M-block) items ...
     lay_c = api.sift_metadata_layout(shape)
     for l in lay:
         s = np.sort(v["sched"][l])
         exp = np.sort(np.array([(h << 20) | mb for h in range(w.shape.n_q_heads) for mb in range(lay_c.n_mblocks)]))
         assert np.array_equal(s, exp)
+        assert_schedule_order(w, v["sched"][l], ref, l)
     return v, ref
+
+
+def assert_schedule_order(w, sched, ref, layer):
+    """... in the order the persistent attention grid relies on: groups of kv
+    heads one after the other (their K/V fit the L2), and inside a group the cost of the items never increases.  The cost
+    is recomputed here from the ORACLE's counts: steps of an M-block (2 consecutive tiles of one segment) = per document
+    tile ceil(cross entries of its document / 128) (G = 1) or the number of listed pages (G = tile), plus its local
+    count; per user-query tile ceil((row0 + rows) / 128)."""
+    sh = w.shape
+    D, T, G, Hq, Hkv = sh.n_docs, sh.tile, sh.cross_gran, sh.n_q_heads, sh.n_kv_heads
+    base, seg, row0, rows = ref["tile_base"], ref["tile_seg"], ref["tile_row0"], ref["tile_rows"]
+    mb_tiles = []                                     # M-block -> its tiles
+    for d in range(D + 1):
+        for t0 in range(int(base[d]), int(base[d + 1]), 2):
+            mb_tiles.append(list(range(t0, min(t0 + 2, int(base[d + 1])))))
+    per_head = sh.n_tokens * sh.head_dim * 2 * 2
+    kv_per_group = int(min(max((72 << 20) // max(per_head, 1), 1), Hkv))
+    groups = -(-Hkv // kv_per_group)
+    cap = 4096 // groups - 1                          # costs are bucketed up to this value
+    last_g, last_c = -1, None
+    for code in sched:
+        h, mb = int(code) >> 20, int(code) & 0xFFFFF
+        c = 0
+        for t in mb_tiles[mb]:
+            d = int(seg[t])
+            if d < D:
+                cp = int(ref["cross_ptr"][layer, h, d])
+                c += (-(-cp // 128) if G == 1 else cp) + int(ref["local_cnt"][layer, h, t])
+            else:
+                c += -(-(int(row0[t]) + int(rows[t])) // 128)
+        c = min(c, cap)
+        g = (h // (Hq // Hkv)) // kv_per_group
+        assert g >= last_g, ("kv-head groups out of order", h, mb)
+        if g != last_g:
+            last_g, last_c = g, None
+        assert last_c is None or c <= last_c, ("cost increases inside a kv-head group", h, mb, c, last_c)
+        last_c = c
 
 
 def attention_errors(w, layer, o_gpu, lse_gpu, heads, rows, dense=False):
