@@ -605,7 +605,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       if (nsteps > 0) {
         mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 303);
         tc_fence_after();
-        const float inv = l > 0.f ? 1.f / l : 0.f;
+        const float inv = (m > -INFINITY) ? 1.f / l : 0.f;   // a row with no allowed key keeps m = -inf (A13)
 #pragma unroll
         for (int c = 0; c < HD / 32; ++c) {
           uint32_t o[32];
@@ -629,7 +629,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         for (int i = 0; i < HD / 8; ++i) *reinterpret_cast<uint4*>(orow + i * 8) = make_uint4(0, 0, 0, 0);
       }
       if (row_ok && p.lse != nullptr)
-        p.lse[(int64_t)h * p.n_tokens + grow] = (l > 0.f) ? (m * sl + log2f(l)) * 0.6931471805599453f : -INFINITY;
+        p.lse[(int64_t)h * p.n_tokens + grow] = (m > -INFINITY) ? (m * sl + log2f(l)) * 0.6931471805599453f : -INFINITY;
     }
     }
   } else {

@@ -44,6 +44,10 @@ enum { kSmemSlotAttn64 = 0, kSmemSlotAttn128, kSmemSlotEnc64, kSmemSlotEnc128, k
 int ensure_dynamic_smem(const void* func, int bytes, int slot);
 
 static inline int ceil_div_i(int a, int b) { return (a + b - 1) / b; }
+// private array behind `counters`: the sort key of every work item, [L][n_items] int32 (compute_layout reserves it)
+static inline size_t sched_key_offset(const sift_md_layout& lay, int n_layers) {
+  return (lay.counters + (size_t)n_layers * 2 * 4 + 127) / 128 * 128;
+}
 
 // How many kv heads the scheduler lets the grid work on at a time: as many as keep their K and V (n_tokens x head_dim
 // bf16 each) within ~72 MB of the 126 MB L2.  Measured on B200: C3 32K is fastest with >= 4 of its 8

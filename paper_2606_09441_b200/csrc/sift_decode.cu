@@ -1,11 +1,14 @@
-// SIFT metadata decode for sm_100a (sec 5.1): bit vectors -> MD-v1 index lists.
+// SIFT metadata decode for sm_100a (sec 5.1): bit vectors -> MD-v1 index lists, ONE launch.
 //
 // The paper launches one 128-thread CTA per (head, M-block) and replicates the CA entries into every
-// M-block's list.  Here one CTA handles a whole (layer, head): the CA entries of a head form ONE ascending
-// list of which document d uses the prefix [0, cross_ptr[d]), so the CA bits are scanned
-// once per head instead of once per M-block.  Pass 1 (count) = popc of masked 32-bit words, offsets = block
-// exclusive scan (warp shuffles), pass 2 (fill) = ffs-compaction of the same registers; the two passes of
-// the paper are fused per 8192-bit chunk so the bit vectors are read from HBM once.
+// M-block's list.  Here the CA entries of a head form ONE ascending list of which document d uses the prefix
+// [0, cross_ptr[d]), so the CA bits are scanned once per head instead of once per M-block.
+// Grid (q-head, layer, role): role < cross_parts = one range of the head's cross list, then the local lists, then
+// (small grids only) the scheduler keys.  Pass 1 (count) = popc of masked 32-bit words, offsets = batched block scan
+// (warp shuffles), pass 2 (fill) = ffs-compaction of the same registers into a warp-private slice of shared memory
+// and a coalesced copy; the two passes of the paper are fused so the bit vectors are read from HBM once.
+// The tile scheduler (a5) is fused as well: every (layer, head) publishes the sort key of its work items, and the
+// CTA that finishes a layer last counting-sorts the layer's items (no second launch).
 //
 // Bit vectors are byte-aligned per (layer, head, doc), not word-aligned: the kernel reads the
 // aligned 32-bit words that cover a vector and masks the lead/tail bits.
@@ -18,18 +21,30 @@ constexpr int kWPT = 4;    // CA words per thread and pass (a pass = 32768 key b
 constexpr int kTPT = 2;    // tiles per thread and pass
 constexpr int kMaxCrossParts = 4;   // CTAs that may share the cross list of one (layer, head) when the grid is small
 constexpr int kStageEntries = 4096;   // shared-memory staging of one chunk: up to 50% of its 8192 bits set
-constexpr int kSchedThreads = 1024;
-constexpr int kCostBuckets = 4096;
+constexpr int kWarpStage = kStageEntries / (kDecodeThreads / 32);   // staging slice of a warp: its 32 words, <= 50% set
+constexpr int kCostBuckets = 4096;    // buckets of the scheduler's counting sort (they reuse the staging buffer)
+static_assert(kCostBuckets == kStageEntries, "the scheduler's (padded) histogram lives in the staging buffer");
+static_assert(kCostBuckets / kDecodeThreads == 16, "histogram padding: one word per 16 buckets");
+
+// "CTAs of this layer that have finished" counters of the fused scheduler: every decode call takes n_layers
+// consecutive slots of this ring; the CTA that finishes a layer last sorts the layer's work items and puts the
+// slot back to 0, so the ring is all-zero whenever no decode is in flight.
+constexpr int kDoneRing = 1 << 16;
+__device__ int32_t g_layer_done[kDoneRing];
+static std::atomic<uint32_t> g_done_ticket{0};
 
 struct DecodeParams {
   const uint8_t* la;
   const uint8_t* ca;
   int32_t *tile_base, *tile_seg, *tile_row0, *tile_rows;
   int32_t *cross_ptr, *cross_idx, *local_cnt, *local_ptr, *local_idx;
-  int32_t *mblock_tile0, *sched, *counters;
+  int32_t *mblock_tile0, *sched, *counters, *sched_key;
   int32_t n_q_heads, n_kv_heads, n_tiles, cross_cap, local_cap, n_mblocks, n_items, gran;
   int32_t kv_per_group;   // kv heads whose work items are scheduled together (sched_kv_heads_per_group)
   int32_t cross_parts;    // CTAs per (layer, head) for the cross list: 4 when the grid would not fill the GPU, else 1
+  int32_t tile_shift, gran_shift;   // tile and cross_gran are powers of two (64 | 128; 1 | tile): no integer divisions
+  int32_t done_base;      // first slot of this call in g_layer_done
+  int32_t split_keys;     // 1: a separate CTA per (layer, head) computes the scheduler keys
 };
 
 // exclusive scan over the block; returns the exclusive prefix of v and (via total) the block sum
@@ -63,11 +78,15 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int* warp_sums /*[THR
 }
 
 // largest d in [0, n) with tab[d] <= x  (tab ascending, tab[0] <= x)
-__device__ __forceinline__ int upper_seg(const int* tab, int n, int x) {
-  int lo = 0, hi = n - 1;
-  while (lo < hi) {
-    int mid = (lo + hi + 1) >> 1;
-    if (tab[mid] <= x) lo = mid; else hi = mid - 1;
+// Predicated probes (no data-dependent branch); top = largest power of two < n (upper_seg_top), so the depth follows the
+// number of documents.
+__device__ __forceinline__ int upper_seg_top(int n) { return n > 1 ? 1 << (31 - __clz(n - 1)) : 0; }
+__device__ __forceinline__ int upper_seg(const int* tab, int n, int x, int top) {
+  int lo = 0;
+  for (int step = top; step > 0; step >>= 1) {
+    const int mid = lo + step;
+    const int v = tab[min(mid, n - 1)];
+    lo = (mid < n && v <= x) ? mid : lo;
   }
   return lo;
 }
@@ -150,12 +169,19 @@ __device__ __forceinline__ int msb_bit(const uint8_t* __restrict__ v, int n) {
 }
 
 __global__ void __launch_bounds__(kDecodeThreads)
-sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
+sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
   __shared__ int s_tile_base[SIFT_MAX_DOCS + 2];
   __shared__ int s_wstart[SIFT_MAX_DOCS + 2];
   __shared__ int s_mb_base[SIFT_MAX_DOCS + 2];
+  // per-document copies of the kernel-parameter table: a per-lane index into the constant bank is replayed once per
+  // distinct address, shared memory is not
+  __shared__ int s_off[SIFT_MAX_DOCS + 2];        // first row of the segment; s_off[D + 1] = n_tokens
+  __shared__ int s_ca_lead[SIFT_MAX_DOCS];        // bit offset of the head's CA vector inside its first covering word
+  __shared__ int64_t s_doc64[2 * SIFT_MAX_DOCS];  // (the scheduler reuses these 8 KB for its bucket cache)
+  int64_t* s_ca_word = s_doc64;                   // index (in 32-bit words from the 4-byte aligned base of p.ca) of that word
+  int64_t* s_la_off = s_doc64 + SIFT_MAX_DOCS;
   __shared__ int s_scan[kDecodeThreads / 32 + 1];
-  __shared__ int s_stage[kStageEntries];   // compacted entries of one 256-word chunk (denser chunks go straight to global)
+  __shared__ int s_stage[kStageEntries + kStageEntries / 16];   // compacted entries of one 256-word chunk (denser chunks go straight to global)
   __shared__ int s_bscan[2][(kWPT > kTPT ? kWPT : kTPT) * (kDecodeThreads / 32)];
 
   const int tid = threadIdx.x;
@@ -165,45 +191,59 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
   constexpr int NQ = SIFT_Q_TILES_PER_ITEM;
 
   // ---- step 0: per-segment tables (tiles, covering words of this head's CA vectors, M-blocks) ----------
-  {
+  // One warp scans the D + 1 segments 32 at a time (three running sums through shuffles); the other warps wait at a
+  // single barrier.  (The first version ran three block-wide scans per 256 segments in every CTA.)
+  const int tsh = p.tile_shift, gsh = p.gran_shift;
+  if (tid < 32) {
     int carry_t = 0, carry_w = 0, carry_m = 0;
-    for (int d0 = 0; d0 <= D; d0 += kDecodeThreads) {
+    for (int d0 = 0; d0 <= D; d0 += 32) {
       const int d = d0 + tid;
       int pd = 0, nw = 0;
       if (d < D) {
-        const int len = dt.off[d + 1] - dt.off[d];
-        pd = (len + T - 1) / T;
-        const int nbits = (len + G - 1) / G;
-        const int64_t a = dt.ca_off[d] + lh * ((nbits + 7) >> 3);
-        const int lead = (int)((reinterpret_cast<uintptr_t>(p.ca) + (uint64_t)a) & 3);
+        const int o0 = dt.off[d], len = dt.off[d + 1] - o0;
+        pd = (len + T - 1) >> tsh;
+        const int nbits = (len + G - 1) >> gsh;
+        const uint64_t a = (reinterpret_cast<uintptr_t>(p.ca) & 3) + (uint64_t)(dt.ca_off[d] + lh * ((nbits + 7) >> 3));
+        const int lead = (int)(a & 3);
         nw = (lead * 8 + nbits + 31) >> 5;
+        s_off[d] = o0; s_ca_lead[d] = lead * 8; s_ca_word[d] = (int64_t)(a >> 2); s_la_off[d] = dt.la_off[d];
       } else if (d == D) {
-        pd = (dt.query_len + T - 1) / T;
+        pd = (dt.query_len + T - 1) >> tsh;
+        s_off[D] = dt.off[D]; s_off[D + 1] = dt.off[D] + dt.query_len;
       }
-      int tot;
-      int et = block_exclusive_scan<kDecodeThreads>(pd, s_scan, tot);
-      if (d <= D) s_tile_base[d] = carry_t + et;
-      carry_t += tot;
-      int ew = block_exclusive_scan<kDecodeThreads>(nw, s_scan, tot);
-      if (d <= D) s_wstart[d] = carry_w + ew;
-      carry_w += tot;
-      int em = block_exclusive_scan<kDecodeThreads>((pd + NQ - 1) / NQ, s_scan, tot);
-      if (d <= D) s_mb_base[d] = carry_m + em;
-      carry_m += tot;
+      int it = pd, iw = nw, im = (pd + NQ - 1) / NQ;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int a = __shfl_up_sync(0xffffffffu, it, o), b = __shfl_up_sync(0xffffffffu, iw, o),
+                  c = __shfl_up_sync(0xffffffffu, im, o);
+        if (tid >= o) { it += a; iw += b; im += c; }
+      }
+      if (d <= D) {
+        s_tile_base[d] = carry_t + it - pd;
+        s_wstart[d] = carry_w + iw - nw;
+        s_mb_base[d] = carry_m + im - (pd + NQ - 1) / NQ;
+      }
+      carry_t += __shfl_sync(0xffffffffu, it, 31);
+      carry_w += __shfl_sync(0xffffffffu, iw, 31);
+      carry_m += __shfl_sync(0xffffffffu, im, 31);
     }
     if (tid == 0) {
       s_tile_base[D + 1] = carry_t;
       s_wstart[D + 1] = carry_w;   // s_wstart[D] == carry_w as well (the query has no CA words)
       s_mb_base[D + 1] = carry_m;
     }
-    __syncthreads();
   }
+  __syncthreads();
   const int NT = s_tile_base[D + 1];
   // blockIdx.z splits a (layer, head): z < kCrossParts = one range of the cross list, z = kCrossParts = the local lists
   // (and, for the first head, the tile tables).  Shortens the latency chain of a CTA (a single layer is latency-bound).
   const int kCrossParts = p.cross_parts;
   const bool do_cross = ((int)blockIdx.z < kCrossParts);
-  const bool writer = (h == 0 && l == 0 && !do_cross);
+  // the scheduler keys of the head come from the local-list CTA, or, when the grid is small (split_keys), from a CTA
+  // of their own (z = kCrossParts + 1) so that the call's critical path is shorter
+  const bool do_local = ((int)blockIdx.z == kCrossParts);
+  const bool do_keys = p.split_keys ? ((int)blockIdx.z == kCrossParts + 1) : do_local;
+  const bool writer = (h == 0 && l == 0 && do_local);
   if (writer) {
     for (int d = tid; d <= D + 1; d += kDecodeThreads) p.tile_base[d] = s_tile_base[d];
     for (int d = tid; d <= D; d += kDecodeThreads) {
@@ -222,14 +262,15 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
   int32_t* cross_idx = p.cross_idx + lh * p.cross_cap;
   // masked stream-order bits of word v of the head's virtual word sequence, the global coordinate of its bit 0 and
   // the document it closes (or -1)
-  auto load_word = [&](int v, int& key0, int& closes) -> uint32_t {
-    const int d = upper_seg(s_wstart, D, v);
+  const int top_d = upper_seg_top(D), top_d1 = upper_seg_top(D + 1);
+  const uint32_t* ca_words = reinterpret_cast<const uint32_t*>(reinterpret_cast<uintptr_t>(p.ca) & ~(uintptr_t)3);
+  auto load_word = [&](int v, int& key0, int& closes, int* doc = nullptr) -> uint32_t {
+    const int d = upper_seg(s_wstart, D, v, top_d);
     const int wi = v - s_wstart[d];
-    const int len = dt.off[d + 1] - dt.off[d];
-    const int nbits = (len + G - 1) / G;
-    const uintptr_t a = reinterpret_cast<uintptr_t>(p.ca) + (uint64_t)(dt.ca_off[d] + lh * ((nbits + 7) >> 3));
-    const int lead = (int)(a & 3) * 8;
-    const uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(a & ~(uintptr_t)3) + wi);
+    const int len = s_off[d + 1] - s_off[d];
+    const int nbits = (len + G - 1) >> gsh;
+    const int lead = s_ca_lead[d];
+    const uint32_t w = __ldg(ca_words + s_ca_word[d] + wi);
     // stream bit s (MSB-first within each byte, bytes ascending) -> bit s of x
     const uint32_t x = __brev(__byte_perm(w, 0, 0x0123));
     const int lo = max(0, lead - wi * 32);
@@ -237,8 +278,9 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
     uint32_t m = (hi >= 32) ? 0xffffffffu : ((1u << hi) - 1u);
     m &= ~((lo >= 32) ? 0xffffffffu : ((1u << lo) - 1u));
     // global coordinate of stream bit 0 of this word: key row (G == 1) or tile id (G == tile; a page is a tile)
-    key0 = (G == 1 ? dt.off[d] : s_tile_base[d]) + wi * 32 - lead;
+    key0 = (G == 1 ? s_off[d] : s_tile_base[d]) + wi * 32 - lead;
     closes = (v + 1 == s_wstart[d + 1]) ? d : -1;
+    if (doc) *doc = d;
     return x & m;
   };
   // The word sequence of a head is cut into kCrossParts ranges, one CTA each (grid z): a CTA first popcounts the words
@@ -251,6 +293,7 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
   int running = 0;
   if (do_cross) {
     int before = 0, k0, cl;
+#pragma unroll 4
     for (int v = tid; v < w_lo; v += kDecodeThreads) before += __popc(load_word(v, k0, cl));
     int tot;
     block_exclusive_scan<kDecodeThreads>(before, s_scan, tot);
@@ -269,29 +312,33 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
     }
 #pragma unroll
     for (int k = 0; k < kWPT; ++k) cnt[k] = __popc(bits[k]);                     // pass 1: count
-    int ex[kWPT], cs[kWPT], ct[kWPT];
-    const int pass_total = batched_exclusive_scan<kWPT>(cnt, ex, s_bscan[scan_no++ & 1], cs, ct);   // offsets
-    // pass 2: fill, global coordinates.  Each 256-word chunk is compacted into shared memory by a thread-per-word
-    // ffs loop and then copied out with coalesced stores: scattering the ffs loop straight to global memory cost 32
-    // sectors per store instruction, a warp-cooperative bit-per-lane fill cost ~1500 instructions per warp and made
-    // the kernel issue-bound (65% issue-active, 56 us for the 32 layers of C5).
+    int ex[kWPT];
+    const int pass_total = batched_exclusive_scan<kWPT>(cnt, ex, s_bscan[scan_no++ & 1]);   // offsets
+    // pass 2: fill, global coordinates.  Every warp compacts its own 32 words with a thread-per-word ffs loop into a
+    // private slice of shared memory and copies the slice out with coalesced stores: no block barrier in the fill (the
+    // first version staged 256 words per block between two __syncthreads, eight barriers per pass), and no scattered
+    // 4-byte stores (32 sectors per store instruction when the ffs loop wrote straight to global memory).
 #pragma unroll
     for (int k = 0; k < kWPT; ++k) {
       if (dd[k] >= 0) cross_ptr[dd[k] + 1] = running + ex[k] + cnt[k];
-      if (ct[k] == 0) continue;                        // block-uniform
-      int32_t* dst = cross_idx + running + cs[k];
-      int o = ex[k] - cs[k];
+      const int lane = tid & 31, wid = tid >> 5;
+      const int wbase = __shfl_sync(0xffffffffu, ex[k], 0);                      // list offset of the warp's first entry
+      const int wtot = __shfl_sync(0xffffffffu, ex[k] + cnt[k], 31) - wbase;     // entries of the warp's 32 words
+      if (wtot == 0) continue;                                                   // warp-uniform
+      int32_t* dst = cross_idx + running + wbase;
+      int o = ex[k] - wbase;
       uint32_t bk = bits[k];
-      if (ct[k] <= kStageEntries) {                    // block-uniform
+      if (wtot <= kWarpStage) {
+        int* stage = s_stage + wid * kWarpStage;
         while (bk) {
           const int sb = __ffs(bk) - 1;
           bk &= bk - 1;
-          s_stage[o++] = key0[k] + sb;
+          stage[o++] = key0[k] + sb;
         }
-        __syncthreads();
-        for (int i = tid; i < ct[k]; i += kDecodeThreads) dst[i] = s_stage[i];
-        __syncthreads();
-      } else {
+        __syncwarp();
+        for (int i = lane; i < wtot; i += 32) dst[i] = stage[i];
+        __syncwarp();
+      } else {                                            // more than half of the warp's 1024 bits set
         while (bk) {
           const int sb = __ffs(bk) - 1;
           bk &= bk - 1;
@@ -305,128 +352,177 @@ sift_decode_lists_kernel(const __grid_constant__ DocTable dt, const DecodeParams
   if (do_cross) {
     if (blockIdx.z == kCrossParts - 1)
       for (int i = running + tid; i < ((running + 127) & ~127); i += kDecodeThreads) cross_idx[i] = 0;
-    return;
-  }
-
-  // ---- local lists: LA row popcounts, offsets, fill -------------------------------------------------
-  int32_t* local_cnt = p.local_cnt + lh * NT;
-  int32_t* local_ptr = p.local_ptr + lh * (NT + 1);
-  int32_t* local_idx = p.local_idx + lh * p.local_cap;
-  running = 0;
-  for (int base = 0; base < NT; base += kTPT * kDecodeThreads) {
-    int cnt[kTPT], dd[kTPT], ii[kTPT];
-    const uint8_t* lv[kTPT];
+  } else if (do_local) {
+    // ---- local lists: LA row popcounts, offsets, fill -------------------------------------------------
+    int32_t* local_cnt = p.local_cnt + lh * NT;
+    int32_t* local_ptr = p.local_ptr + lh * (NT + 1);
+    int32_t* local_idx = p.local_idx + lh * p.local_cap;
+    const int tq0 = s_tile_base[D];          // first tile of the user query
+    running = 0;
+    for (int base = 0; base < NT; base += kTPT * kDecodeThreads) {
+      int cnt[kTPT], dd[kTPT], ii[kTPT];
+      const uint8_t* lv[kTPT];
 #pragma unroll
-    for (int k = 0; k < kTPT; ++k) {
-      const int t = base + k * kDecodeThreads + tid;
-      cnt[k] = 0; dd[k] = 0; ii[k] = 0; lv[k] = nullptr;
-      if (t < NT) {
-        const int d = upper_seg(s_tile_base, D + 1, t);
-        const int i = t - s_tile_base[d];
-        dd[k] = d; ii[k] = i;
-        const int seg_len = (d < D) ? dt.off[d + 1] - dt.off[d] : dt.query_len;
-        if (writer) {
-          p.tile_seg[t] = d;
-          p.tile_row0[t] = dt.off[d] + i * T;
-          p.tile_rows[t] = min(T, seg_len - i * T);
-        }
-        if (d == D) {
-          cnt[k] = t + 1;                                             // query M-block: all causal N-blocks (L243)
-        } else {
-          const int pd = s_tile_base[d + 1] - s_tile_base[d];
-          const int nbytes = (pd * (pd + 1) / 2 + 7) >> 3;
-          lv[k] = p.la + dt.la_off[d] + lh * nbytes;
-          cnt[k] = la_row_count(lv[k], i);
-        }
-      }
-    }
-    int ex[kTPT];
-    const int pass_total = batched_exclusive_scan<kTPT>(cnt, ex, s_bscan[scan_no++ & 1]);
-#pragma unroll
-    for (int k = 0; k < kTPT; ++k) {
-      const int t = base + k * kDecodeThreads + tid;
-      if (t < NT) {
-        int w0 = running + ex[k];
-        local_cnt[t] = cnt[k];
-        local_ptr[t] = w0;
-        if (dd[k] == D) {
-          for (int j = 0; j <= t; ++j) local_idx[w0 + j] = j;
-        } else {
-          la_row_fill(lv[k], ii[k], s_tile_base[dd[k]], local_idx + w0);
+      for (int k = 0; k < kTPT; ++k) {
+        const int t = base + k * kDecodeThreads + tid;
+        cnt[k] = 0; dd[k] = 0; ii[k] = 0; lv[k] = nullptr;
+        if (t < NT) {
+          const int d = upper_seg(s_tile_base, D + 1, t, top_d1);
+          const int i = t - s_tile_base[d];
+          dd[k] = d; ii[k] = i;
+          const int seg_len = s_off[d + 1] - s_off[d];
+          if (writer) {
+            p.tile_seg[t] = d;
+            p.tile_row0[t] = s_off[d] + i * T;
+            p.tile_rows[t] = min(T, seg_len - i * T);
+          }
+          if (d == D) {
+            cnt[k] = t + 1;                                             // query M-block: all causal N-blocks (L243)
+          } else {
+            const int pd = s_tile_base[d + 1] - s_tile_base[d];
+            const int nbytes = (pd * (pd + 1) / 2 + 7) >> 3;
+            lv[k] = p.la + s_la_off[d] + lh * nbytes;
+            cnt[k] = la_row_count(lv[k], i);
+          }
         }
       }
+      int ex[kTPT];
+      const int pass_total = batched_exclusive_scan<kTPT>(cnt, ex, s_bscan[scan_no++ & 1]);
+#pragma unroll
+      for (int k = 0; k < kTPT; ++k) {
+        const int t = base + k * kDecodeThreads + tid;
+        if (t < NT) {
+          const int w0 = running + ex[k];
+          local_cnt[t] = cnt[k];
+          local_ptr[t] = w0;
+          if (t == tq0) s_scan[0] = w0;      // where the query tiles' lists start (filled by the whole block below)
+          if (dd[k] < D) la_row_fill(lv[k], ii[k], s_tile_base[dd[k]], local_idx + w0);
+        }
+      }
+      running += pass_total;
     }
-    running += pass_total;
+    if (tid == 0) local_ptr[NT] = running;
+    __syncthreads();
+    // query tile t lists all causal tiles 0 .. t: written by the whole block with coalesced stores (one thread per
+    // tile wrote up to ~500 entries one after the other in the first version)
+    {
+      int w0 = s_scan[0];
+      for (int t = tq0; t < NT; ++t) {
+        for (int j = tid; j <= t; j += kDecodeThreads) local_idx[w0 + j] = j;
+        w0 += t + 1;
+      }
+    }
   }
-  if (tid == 0) local_ptr[NT] = running;
-}
+  if (do_keys) {
+    // ---- scheduler keys of this head's work items (a5).  key = processing order: groups of kv heads one after the
+    // other (the q-heads of a kv head gather from the same K/V, so the K/V working set of the grid stays L2-sized and
+    // K/V are read from HBM about once), longest items first inside a group.  cost = steps of the item's tiles: groups
+    // of 128 gathered rows (G == 1) or one page per step (G == tile) + local tiles | dense steps of query tiles.
+    // The counts are recounted here from the bits (a few KB, read by the list CTAs at the same time) instead of waiting
+    // for the lists: every CTA of the layer only publishes, and the CTA that finishes last just sorts the keys.
+    {
+      __syncthreads();                                         // (the local lists above are done with s_stage / s_scan)
+      int* s_ccnt = s_stage;                                   // [D + 1]: entries in documents < d
+      for (int d = tid; d <= D; d += kDecodeThreads) s_ccnt[d] = 0;
+      __syncthreads();
+#pragma unroll 4
+      for (int v = tid; v < all_words; v += kDecodeThreads) {
+        int k0, cl, d;
+        const int c = __popc(load_word(v, k0, cl, &d));
+        if (c) atomicAdd(&s_ccnt[d + 1], c);
+      }
+      __syncthreads();
+      if (tid < 32) {
+        int carry = 0;
+        for (int d0 = 0; d0 <= D; d0 += 32) {
+          const int d = d0 + tid;
+          int v = (d <= D) ? s_ccnt[d] : 0;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            const int n = __shfl_up_sync(0xffffffffu, v, o);
+            if (tid >= o) v += n;
+          }
+          if (d <= D) s_ccnt[d] = carry + v;
+          carry += __shfl_sync(0xffffffffu, v, 31);
+        }
+      }
+      __syncthreads();
+      const int groups = (p.n_kv_heads + p.kv_per_group - 1) / p.kv_per_group, bpg = kCostBuckets / groups;
+      const int g = h / ((p.n_q_heads / p.n_kv_heads) * p.kv_per_group);
+      int32_t* key = p.sched_key + (int64_t)l * p.n_items + (int64_t)h * p.n_mblocks;
+      static_assert(NQ == 2, "cost of an M-block: two tiles");
+      for (int mb = tid; mb < p.n_mblocks; mb += kDecodeThreads) {
+        const int seg = upper_seg(s_mb_base, D + 1, mb, top_d1);
+        const int t0 = s_tile_base[seg] + (mb - s_mb_base[seg]) * NQ;
+        const bool two = t0 + 1 < s_tile_base[seg + 1];
+        int c;
+        if (seg < D) {
+          const int cp = s_ccnt[seg];
+          const int cross_steps = (G == 1) ? (cp + 127) >> 7 : cp;
+          const int pd = s_tile_base[seg + 1] - s_tile_base[seg], i0 = t0 - s_tile_base[seg];
+          const uint8_t* lv = p.la + s_la_off[seg] + lh * ((pd * (pd + 1) / 2 + 7) >> 3);
+          c = (two ? 2 : 1) * cross_steps + la_row_count(lv, i0) + (two ? la_row_count(lv, i0 + 1) : 0);
+        } else {
+          const int r0 = s_off[D] + (t0 - s_tile_base[D]) * T;     // dense steps of the query tiles: keys 0 .. last row
+          c = (min(r0 + T, s_off[D + 1]) + 127) >> 7;
+          if (two) c += (min(r0 + 2 * T, s_off[D + 1]) + 127) >> 7;
+        }
+        key[mb] = g * bpg + (bpg - 1 - min(c, bpg - 1));
+      }
+    }
+  }
 
-// Work items (head, M-block) of one layer sorted by (kv-head group, descending cost) (counting sort): the persistent
-// attention grid pulls them through an atomic counter.
-__global__ void __launch_bounds__(kSchedThreads)
-sift_schedule_kernel(const DecodeParams p, int n_docs, int n_layers_unused) {
-  __shared__ int s_hist[kCostBuckets];
-  __shared__ int s_scan[kSchedThreads / 32 + 1];
-  constexpr int NQ = SIFT_Q_TILES_PER_ITEM;
-  const int l = blockIdx.x, tid = threadIdx.x;
-  const int D = n_docs, NT = p.n_tiles, NMB = p.n_mblocks;
-  for (int i = tid; i < kCostBuckets; i += kSchedThreads) s_hist[i] = 0;
+  // ---- scheduler (a5), fused: the CTA that finishes a layer last sorts the layer's work items (head, M-block) by
+  // key = (kv-head group, descending cost) with a counting sort in shared memory; the persistent attention grid pulls
+  // them through an atomic counter.  The keys of the other CTAs are published by the fence + counter below.
+  __shared__ int s_last;
+  __threadfence();
   __syncthreads();
-  auto cost_of = [&](int e) {
-    const int h = e / NMB, mb = e - h * NMB;
-    const int64_t lh = (int64_t)l * p.n_q_heads + h;
-    const int t0 = p.mblock_tile0[mb], t1 = min(p.mblock_tile0[mb + 1], t0 + NQ);
-    const int seg = p.tile_seg[t0];
-    int c = 0;
-    for (int t = t0; t < t1; ++t) {
-      // steps of a document tile: groups of 128 gathered rows (G == 1) or one page per step (G == tile), plus local tiles
-      if (seg < D) c += (p.gran == 1 ? (p.cross_ptr[lh * (D + 1) + seg] + 127) / 128 : p.cross_ptr[lh * (D + 1) + seg]) + p.local_cnt[lh * NT + t];
-      else c += (p.tile_row0[t] + p.tile_rows[t] + 127) / 128;
+  int32_t* done = &g_layer_done[(uint32_t)(p.done_base + l) % kDoneRing];
+  if (tid == 0) s_last = (atomicAdd(done, 1) == (int)(gridDim.x * gridDim.z) - 1);
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  {
+    int* s_hist = s_stage;
+    const int NMB = p.n_mblocks;
+    auto hx = [](int b) { return b + (b >> 4); };   // 16 consecutive buckets per thread in the scan: pad against bank conflicts
+    for (int i = tid; i < kCostBuckets + kCostBuckets / 16; i += kDecodeThreads) s_hist[i] = 0;
+    __syncthreads();
+    // The sort runs once per layer, in a CTA that is alone on its SM, right after the L1 was invalidated: its code is
+    // fetched cold.  So it is written as small loops (a 17x unrolled version spent 40K+ cycles on instruction fetch),
+    // unrolled by 4 so that the loads of four items overlap.  Thread t owns items t*per .. t*per+per-1:
+    // the items of a warp instruction are `per` apart (other documents, other costs), so its lanes seldom hit the same
+    // histogram bucket (consecutive M-blocks of a head mostly do).
+    const int32_t* key = p.sched_key + (int64_t)l * p.n_items;   // (plain loads: the fence above invalidated this SM's L1)
+    const int n_items = p.n_items;
+    const int per = (n_items + kDecodeThreads - 1) / kDecodeThreads, e0 = tid * per, e1 = min(n_items, e0 + per);
+#pragma unroll 4
+    for (int e = e0; e < e1; ++e) {
+      atomicAdd(&s_hist[hx(key[e])], 1);
     }
-    // bucket = processing order: groups of kv heads one after the other (the q-heads of a kv head gather from the same
-    // K/V, so the K/V working set of the grid stays L2-sized and K/V are read from HBM about once), longest items
-    // first inside a group
-    const int groups = (p.n_kv_heads + p.kv_per_group - 1) / p.kv_per_group, bpg = kCostBuckets / groups;
-    const int g = h / (p.n_q_heads / p.n_kv_heads) / p.kv_per_group;
-    return g * bpg + (bpg - 1 - min(c, bpg - 1));
-  };
-  // the cost of an item is a chain of dependent global loads: evaluate it once and keep it in registers for the
-  // scatter pass (up to kCached items per thread; larger layers recompute)
-  constexpr int kCached = 8;
-  int ccost[kCached];
-#pragma unroll
-  for (int k = 0; k < kCached; ++k) {
-    const int e = tid + k * kSchedThreads;
-    ccost[k] = (e < p.n_items) ? cost_of(e) : 0;
+    __syncthreads();
+    {  // exclusive scan over buckets (bucket 0 = first to be processed)
+      constexpr int PER = kCostBuckets / kDecodeThreads;
+      int sum = 0;
+#pragma unroll 4
+      for (int k = 0; k < PER; ++k) sum += s_hist[hx(tid * PER + k)];
+      int tot;
+      int ex = block_exclusive_scan<kDecodeThreads>(sum, s_scan, tot);
+#pragma unroll 4
+      for (int k = 0; k < PER; ++k) { const int c = s_hist[hx(tid * PER + k)]; s_hist[hx(tid * PER + k)] = ex; ex += c; }
+    }
+    __syncthreads();
+    int32_t* sched = p.sched + (int64_t)l * n_items;
+#pragma unroll 4
+    for (int e = e0; e < e1; ++e) {
+      const int b = key[e];
+      const int h2 = e / NMB;
+      sched[atomicAdd(&s_hist[hx(b)], 1)] = (h2 << 20) | (e - h2 * NMB);
+    }
+    if (tid < 2) p.counters[l * 2 + tid] = 0;
+    if (tid == 0) *done = 0;
   }
-#pragma unroll
-  for (int k = 0; k < kCached; ++k)
-    if (tid + k * kSchedThreads < p.n_items) atomicAdd(&s_hist[ccost[k]], 1);
-  for (int e = tid + kCached * kSchedThreads; e < p.n_items; e += kSchedThreads)
-    atomicAdd(&s_hist[cost_of(e)], 1);
-  __syncthreads();
-  {  // exclusive scan over buckets (bucket 0 = first to be processed)
-    constexpr int PER = kCostBuckets / kSchedThreads;
-    int loc[PER], sum = 0;
-#pragma unroll
-    for (int k = 0; k < PER; ++k) { loc[k] = s_hist[tid * PER + k]; sum += loc[k]; }
-    int tot;
-    int ex = block_exclusive_scan<kSchedThreads>(sum, s_scan, tot);
-#pragma unroll
-    for (int k = 0; k < PER; ++k) { s_hist[tid * PER + k] = ex; ex += loc[k]; }
-  }
-  __syncthreads();
-  int32_t* sched = p.sched + (int64_t)l * p.n_items;
-  auto place = [&](int e, int c) {
-    const int h = e / NMB, mb = e - h * NMB;
-    const int pos = atomicAdd(&s_hist[c], 1);
-    sched[pos] = (h << 20) | mb;
-  };
-#pragma unroll
-  for (int k = 0; k < kCached; ++k)
-    if (tid + k * kSchedThreads < p.n_items) place(tid + k * kSchedThreads, ccost[k]);
-  for (int e = tid + kCached * kSchedThreads; e < p.n_items; e += kSchedThreads) place(e, cost_of(e));
-  if (tid < 2) p.counters[l * 2 + tid] = 0;
 }
 
 int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable& dt, const uint8_t* la_base,
@@ -442,6 +538,7 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   p.cross_ptr = at(lay.cross_ptr); p.cross_idx = at(lay.cross_idx);
   p.local_cnt = at(lay.local_cnt); p.local_ptr = at(lay.local_ptr); p.local_idx = at(lay.local_idx);
   p.mblock_tile0 = at(lay.mblock_tile0); p.sched = at(lay.sched); p.counters = at(lay.counters);
+  p.sched_key = at(sched_key_offset(lay, s->n_layers));
   p.n_q_heads = s->n_q_heads; p.n_kv_heads = s->n_kv_heads; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap; p.local_cap = lay.local_cap;
   p.n_mblocks = lay.n_mblocks; p.n_items = lay.n_items; p.gran = s->cross_gran;
   // few (layer, head) pairs (one layer of an 8B-class model = 32): the call is latency-bound, cut each head's cross list
@@ -449,13 +546,17 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   int num_sms = 0;
   if (int rc = device_sm_count(&num_sms)) return rc;
   p.cross_parts = ((int64_t)s->n_q_heads * s->n_layers <= num_sms) ? kMaxCrossParts : 1;
+  p.split_keys = (p.cross_parts > 1);
   p.kv_per_group = sched_kv_heads_per_group((int64_t)s->doc_offsets[s->n_docs] + s->query_len, s->head_dim, s->n_kv_heads);
+  p.tile_shift = (s->tile == 128) ? 7 : 6;
+  p.gran_shift = (s->cross_gran == 1) ? 0 : p.tile_shift;
+  if (s->n_layers > kDoneRing / 4) return set_error(SIFT_ERR_UNSUPPORTED, "too many layers in one decode call");
+  p.done_base = (int32_t)(g_done_ticket.fetch_add((uint32_t)s->n_layers, std::memory_order_relaxed) % kDoneRing);
   cudaGetLastError();
-  sift_decode_lists_kernel<<<dim3(s->n_q_heads, s->n_layers, p.cross_parts + 1), kDecodeThreads, 0, st>>>(dt, p);
-  sift_schedule_kernel<<<s->n_layers, kSchedThreads, 0, st>>>(p, s->n_docs, s->n_layers);
+  sift_decode_kernel<<<dim3(s->n_q_heads, s->n_layers, p.cross_parts + 1 + p.split_keys), kDecodeThreads, 0, st>>>(dt, p);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "decode launch: %s", cudaGetErrorString(e));
-  count_launch(2);
+  count_launch(1);
   return SIFT_OK;
 }
 

@@ -152,6 +152,7 @@ int compute_layout(const sift_shape* s, sift_md_layout* out) {
   out->mblock_tile0 = take(nmb + 1);
   out->sched = take((int64_t)s->n_layers * out->n_items);
   out->counters = take((int64_t)s->n_layers * 2);
+  take((int64_t)s->n_layers * out->n_items);   // scheduler keys (private, unnamed: sched_key_offset())
   out->total_bytes = o;
   return SIFT_OK;
 }
