@@ -16,6 +16,9 @@ What it is: the plain definitions, written out.
                                     (sec 5.1), in the container "MD-v1"
                                     (SURVEY.md 8(c) Part 3; the paper fixes no container).
   Sizes   ``la_vector_bytes`` .. -- PAPER.md:L213 sec 4.3 and Table 1 (L311-321).
+  Part 4  ``encode_document``    -- offline metadata generation (L201, L209, L223).
+  Part 5  ``*_batch``            -- several prompts in one call: a loop over prompts around Parts 1-3, shifted to
+                                    batch coordinates (container "MD-v1b").
 
 Readings of the paper where it is silent or garbled are listed in DESIGN.md section 3
 (A1..A26 of SURVEY.md 8(c)); the ones used here are cited inline.
@@ -23,9 +26,10 @@ Readings of the paper where it is silent or garbled are listed in DESIGN.md sect
 Pins (tests/test_oracle_pins.py): byte patterns from the enumeration printed at L203, the
 P=8 -> 36/8 bits example (L213), all of Table 1, all-ones == dense causal, CA cleared ==
 block diagonal + dense query, brute-force fp64 softmax on tiny inputs, the torch SDPA
-special case, metadata -> mask round trip, reorder invariance.
-Parity unpinned by the paper: the MD-v1 *container layout* (our definition; pinned only by
-the round trip).
+special case, metadata -> mask round trip, reorder invariance; batch: one prompt == MD-v1, block-diagonal mask,
+MD-v1b -> mask round trip, brute force over the packed K/V.
+Parity unpinned by the paper: the MD-v1 / MD-v1b *container layouts* (our definition; pinned only by
+the round trips).
 """
 from __future__ import annotations
 
@@ -410,6 +414,179 @@ def marked_pairs(doc_offsets: Sequence[int], query_len: int, tile: int, gran: in
         rows = list(range(r0, min(n, r0 + block)))
         tot += int(expand_mask_rows(doc_offsets, query_len, tile, gran, la_vecs, ca_vecs, rows).sum())
     return tot
+
+
+# ------------------------------------------------------------------------------------------
+# Part 5: several prompts in one call (sec 2 "TTFT gates decode batching", L267 sec 6)
+# ------------------------------------------------------------------------------------------
+# Plain definition: the prompts are packed back to back on the token axis (prompt p = its documents, then its query);
+# a row of prompt p sees keys of prompt p only, by the single-prompt rule of Part 1.  Everything below is a loop over
+# prompts around Parts 1-3 plus a shift to batch coordinates.  Container "MD-v1b" (ours, like MD-v1; for one prompt it
+# IS MD-v1): segments are numbered in token order (documents and queries alike), documents are numbered in token order,
+#   seg_doc[s]   document index of segment s, -1 for a query segment;  seg_first[s]  first segment of s's prompt
+#   tile_base[S+1], tile_seg / tile_row0 / tile_rows [NT]               as in MD-v1, batch coordinates
+#   cross_ptr[L][H][D+1]  running number of marked keys over the documents in token order, EXCEPT that the list of
+#                         every prompt starts at a multiple of 128 (the attention kernel reads whole groups of 128
+#                         entries): document d of a prompt whose first document is d0 attends entries
+#                         [cross_ptr[d0], cross_ptr[d]); entries between a prompt's end and the next start: unspecified
+#   local_*               per global tile; the list of query tile t of a prompt whose first tile is f is f .. t
+# A prompt is given as (doc_offsets, query_len) with its own offsets starting at 0; vectors are addressed by the
+# document's index in the batch.
+
+Prompt = Tuple[Sequence[int], int]
+
+
+def batch_layout(prompts: Sequence[Prompt], tile: int) -> Dict[str, list]:
+    """row / document / segment / tile base of every prompt, and the segment tables of MD-v1b."""
+    row_base, doc_base, seg_base, tile0 = [0], [0], [0], [0]
+    seg_doc, seg_first, seg_off = [], [], [0]
+    for off, qlen in prompts:
+        off = [int(x) for x in off]
+        n_docs = len(off) - 1
+        tt = tile_tables(off, qlen, tile)
+        for d in range(n_docs):
+            seg_doc.append(doc_base[-1] + d)
+            seg_first.append(seg_base[-1])
+            seg_off.append(row_base[-1] + off[d + 1])
+        seg_doc.append(-1)
+        seg_first.append(seg_base[-1])
+        seg_off.append(row_base[-1] + off[-1] + qlen)
+        row_base.append(row_base[-1] + off[-1] + qlen)
+        doc_base.append(doc_base[-1] + n_docs)
+        seg_base.append(seg_base[-1] + n_docs + 1)
+        tile0.append(tile0[-1] + int(tt["NT"]))
+    return {"row_base": row_base, "doc_base": doc_base, "seg_base": seg_base, "tile0": tile0,
+            "seg_doc": seg_doc, "seg_first": seg_first, "seg_off": seg_off}
+
+
+def prompt_of_row(row: int, row_base: Sequence[int]) -> int:
+    for p in range(len(row_base) - 1):
+        if row_base[p] <= row < row_base[p + 1]:
+            return p
+    raise ValueError("row outside the batch")
+
+
+def expand_mask_rows_batch(prompts: Sequence[Prompt], tile: int, gran: int, la_vecs: Sequence[np.ndarray],
+                           ca_vecs: Sequence[np.ndarray], rows: Sequence[int]) -> np.ndarray:
+    """bool [len(rows), N_total] for one (layer, head); la_vecs / ca_vecs are indexed by the document's batch index."""
+    lay = batch_layout(prompts, tile)
+    out = np.zeros((len(rows), lay["row_base"][-1]), dtype=bool)
+    for ri, q in enumerate(rows):
+        p = prompt_of_row(int(q), lay["row_base"])
+        off, qlen = prompts[p]
+        b, d0, d1 = lay["row_base"][p], lay["doc_base"][p], lay["doc_base"][p + 1]
+        m = expand_mask_rows(off, qlen, tile, gran, la_vecs[d0:d1], ca_vecs[d0:d1], [int(q) - b])
+        out[ri, b: b + m.shape[1]] = m[0]
+    return out
+
+
+def decode_metadata_batch(prompts: Sequence[Prompt], tile: int, gran: int, n_layers: int, n_heads: int,
+                          la_vec: VecFn, ca_vec: VecFn) -> Dict[str, np.ndarray]:
+    """MD-v1b: every prompt decoded on its own (Part 3), then shifted to batch coordinates."""
+    lay = batch_layout(prompts, tile)
+    n_docs, nt = lay["doc_base"][-1], lay["tile0"][-1]
+    parts = []
+    for p, (off, qlen) in enumerate(prompts):
+        d0 = lay["doc_base"][p]
+        parts.append(decode_metadata(off, qlen, tile, gran, n_layers, n_heads,
+                                     lambda l, h, d, d0=d0: la_vec(l, h, d0 + d),
+                                     lambda l, h, d, d0=d0: ca_vec(l, h, d0 + d)))
+    ccap = sum(int(m["cross_cap"]) for m in parts)          # each prompt's list padded to whole groups of 128
+    lcap = 0
+    for p, m in enumerate(parts):                           # query tile t of a prompt lists its own tiles only
+        npd = len(prompts[p][0]) - 1
+        lcap += sum(int(x) * (int(x) + 1) // 2 for x in m["P"][:npd])
+        lcap += sum(t + 1 for t in range(int(m["tile_base"][npd]), int(m["NT"])))
+    cross_ptr = np.zeros((n_layers, n_heads, n_docs + 1), np.int32)
+    cross_idx = np.full((n_layers, n_heads, max(ccap, 128)), -1, np.int32)
+    local_cnt = np.zeros((n_layers, n_heads, nt), np.int32)
+    local_ptr = np.zeros((n_layers, n_heads, nt + 1), np.int32)
+    local_idx = np.full((n_layers, n_heads, max(lcap, 1)), -1, np.int32)
+    tile_base, tile_seg, tile_row0, tile_rows = [0], [], [], []
+    for p, m in enumerate(parts):
+        npd = len(prompts[p][0]) - 1
+        tile_base += [lay["tile0"][p] + int(x) for x in m["tile_base"][1:npd + 2]]
+        tile_seg += [lay["seg_base"][p] + int(x) for x in m["tile_seg"]]
+        tile_row0 += [lay["row_base"][p] + int(x) for x in m["tile_row0"]]
+        tile_rows += [int(x) for x in m["tile_rows"]]
+    for l in range(n_layers):
+        for h in range(n_heads):
+            cstart, lstart = 0, 0
+            for p, m in enumerate(parts):
+                npd = len(prompts[p][0]) - 1
+                d0, t0, rb = lay["doc_base"][p], lay["tile0"][p], lay["row_base"][p]
+                cstart = -(-cstart // 128) * 128                      # a prompt's list starts at a multiple of 128
+                if npd > 0:
+                    cross_ptr[l, h, d0: d0 + npd + 1] = cstart + m["cross_ptr"][l, h]
+                tot = int(m["cross_ptr"][l, h, npd])
+                cross_idx[l, h, cstart: cstart + tot] = m["cross_idx"][l, h, :tot] + (rb if gran == 1 else t0)
+                cstart += tot
+                ntp = int(m["NT"])
+                local_cnt[l, h, t0: t0 + ntp] = m["local_cnt"][l, h]
+                local_ptr[l, h, t0: t0 + ntp + 1] = lstart + m["local_ptr"][l, h]
+                nl = int(m["local_ptr"][l, h, ntp])
+                local_idx[l, h, lstart: lstart + nl] = m["local_idx"][l, h, :nl] + t0
+                lstart += nl
+            cross_ptr[l, h, n_docs] = cstart
+    return {"seg_doc": np.asarray(lay["seg_doc"], np.int32), "seg_first": np.asarray(lay["seg_first"], np.int32),
+            "tile_base": np.asarray(tile_base, np.int32), "NT": nt, "tile_seg": np.asarray(tile_seg, np.int32),
+            "tile_row0": np.asarray(tile_row0, np.int32), "tile_rows": np.asarray(tile_rows, np.int32),
+            "cross_ptr": cross_ptr, "cross_idx": cross_idx, "local_cnt": local_cnt, "local_ptr": local_ptr,
+            "local_idx": local_idx, "cross_cap": max(ccap, 128), "local_cap": max(lcap, 1)}
+
+
+def metadata_batch_to_mask_rows(md: Dict[str, np.ndarray], prompts: Sequence[Prompt], tile: int, gran: int,
+                                layer: int, head: int, rows: Sequence[int]) -> np.ndarray:
+    """Inverse of MD-v1b, written against the container's own rules (not against Part 3): round-trip pin."""
+    lay = batch_layout(prompts, tile)
+    seg_off, seg_doc, seg_first = lay["seg_off"], md["seg_doc"], md["seg_first"]
+    row0, nrows, base = md["tile_row0"], md["tile_rows"], md["tile_base"]
+    out = np.zeros((len(rows), seg_off[-1]), bool)
+    for ri, q in enumerate(rows):
+        q = int(q)
+        s = max(i for i in range(len(seg_off) - 1) if seg_off[i] <= q)
+        while seg_off[s + 1] <= q:          # (zero-length segments share a start row)
+            s += 1
+        t = int(base[s]) + (q - seg_off[s]) // tile
+        d = int(seg_doc[s])
+        if d >= 0:
+            d0 = int(seg_doc[int(seg_first[s])])
+            lo, hi = int(md["cross_ptr"][layer, head, d0]), int(md["cross_ptr"][layer, head, d])
+            assert lo % 128 == 0
+            for e in md["cross_idx"][layer, head, lo:hi]:
+                e = int(e)
+                if gran == 1:
+                    out[ri, e] = True
+                else:
+                    out[ri, int(row0[e]): int(row0[e]) + int(nrows[e])] = True
+        lo, hi = int(md["local_ptr"][layer, head, t]), int(md["local_ptr"][layer, head, t + 1])
+        for e in md["local_idx"][layer, head, lo:hi]:
+            e = int(e)
+            out[ri, int(row0[e]): min(int(row0[e]) + int(nrows[e]), q + 1)] = True
+    return out
+
+
+def sift_attention_rows_batch(q: torch.Tensor, k: torch.Tensor, v: torch.Tensor, head: int, prompts: Sequence[Prompt],
+                              tile: int, gran: int, la_vecs: Sequence[np.ndarray], ca_vecs: Sequence[np.ndarray],
+                              rows: Sequence[int], scale: Optional[float] = None,
+                              dtype: torch.dtype = torch.float32) -> Tuple[torch.Tensor, torch.Tensor]:
+    """(O [len(rows), d], LSE [len(rows)]) for rows of the packed batch: every row is computed inside its own prompt
+    (slices of Q/K/V and of the vectors handed to Part 2's single-prompt routine)."""
+    lay = batch_layout(prompts, tile)
+    rows = [int(r) for r in rows]
+    o_out = torch.zeros((len(rows), q.shape[2]), dtype=dtype)
+    l_out = torch.zeros((len(rows),), dtype=dtype)
+    for p, (off, qlen) in enumerate(prompts):
+        b, e = lay["row_base"][p], lay["row_base"][p + 1]
+        sel = [i for i, r in enumerate(rows) if b <= r < e]
+        if not sel:
+            continue
+        d0, d1 = lay["doc_base"][p], lay["doc_base"][p + 1]
+        o, lse = sift_attention_rows(q[b:e], k[b:e], v[b:e], head, off, qlen, tile, gran, la_vecs[d0:d1], ca_vecs[d0:d1],
+                                     [rows[i] - b for i in sel], scale=scale, dtype=dtype)
+        o_out[sel] = o
+        l_out[sel] = lse
+    return o_out, l_out
 
 
 # ------------------------------------------------------------------------------------------

@@ -330,6 +330,84 @@ def stack_orderings(w: Workload, n: int = 4) -> List[List[int]]:
     return out
 
 
+@dataclass
+class BatchWorkload:
+    """Several prompts packed back to back on the token axis: prompt p = its documents, then its
+    query.  Input plumbing only: the members' blobs are concatenated and their byte offsets shifted."""
+    name: str
+    members: Tuple[Workload, ...]
+
+    def __post_init__(self):
+        m0 = self.members[0].shape
+        for w in self.members:
+            sh = w.shape
+            assert (sh.n_layers, sh.n_q_heads, sh.n_kv_heads, sh.head_dim, sh.tile, sh.cross_gran) == \
+                   (m0.n_layers, m0.n_q_heads, m0.n_kv_heads, m0.head_dim, m0.tile, m0.cross_gran)
+        la_base = np.cumsum([0] + [len(w.la_blob) for w in self.members])
+        ca_base = np.cumsum([0] + [len(w.ca_blob) for w in self.members])
+        self.la_blob = np.concatenate([w.la_blob for w in self.members] + [np.zeros(4, np.uint8)])
+        self.ca_blob = np.concatenate([w.ca_blob for w in self.members] + [np.zeros(4, np.uint8)])
+        self.la_doc_off = np.concatenate([w.la_doc_off + la_base[i] for i, w in enumerate(self.members)]).astype(np.int64)
+        self.ca_doc_off = np.concatenate([w.ca_doc_off + ca_base[i] for i, w in enumerate(self.members)]).astype(np.int64)
+        self.doc_base = np.cumsum([0] + [w.shape.n_docs for w in self.members]).astype(np.int64)
+
+    # -- what the library is told ---------------------------------------------------------------
+    @property
+    def head_shape(self) -> PromptShape:
+        return self.members[0].shape
+
+    @property
+    def doc_lens(self) -> Tuple[int, ...]:
+        return tuple(x for w in self.members for x in w.shape.doc_lens)
+
+    @property
+    def prompt_doc_start(self) -> np.ndarray:
+        return self.doc_base.astype(np.int32)
+
+    @property
+    def prompt_query_len(self) -> np.ndarray:
+        return np.asarray([w.shape.query_len for w in self.members], np.int32)
+
+    @property
+    def n_tokens(self) -> int:
+        return int(sum(w.shape.n_tokens for w in self.members))
+
+    @property
+    def row_base(self) -> np.ndarray:
+        return np.cumsum([0] + [w.shape.n_tokens for w in self.members]).astype(np.int64)
+
+    # -- what the oracle is told -------------------------------------------------------------------
+    @property
+    def prompts(self):
+        return [([int(x) for x in w.shape.doc_offsets], w.shape.query_len) for w in self.members]
+
+    def _member_of_doc(self, d: int):
+        p = int(np.searchsorted(self.doc_base, d, side="right")) - 1
+        return self.members[p], d - int(self.doc_base[p])
+
+    def la_vec(self, layer: int, head: int, d: int) -> np.ndarray:
+        w, pos = self._member_of_doc(d)
+        return w.la_vec(layer, head, pos)
+
+    def ca_vec(self, layer: int, head: int, d: int) -> np.ndarray:
+        w, pos = self._member_of_doc(d)
+        return w.ca_vec(layer, head, pos)
+
+    def qkv(self, layer: int) -> Tuple[torch.Tensor, torch.Tensor, torch.Tensor]:
+        parts = [w.qkv(layer) for w in self.members]
+        return tuple(torch.cat([p[i] for p in parts]) for i in range(3))
+
+
+def make_batch(name: str, members: Sequence[Workload]) -> BatchWorkload:
+    return BatchWorkload(name, tuple(members))
+
+
+def config_batch_8x10k(seed: int = BASE_SEED) -> BatchWorkload:
+    """Eight prompts of C2's shape (10 x 1024 + 128, 32/8 heads, d = 128), different seeds: the multi-request case of
+    SURVEY.md 8(f)-3 (short prompts in one launch fill the GPU where one of them cannot)."""
+    return make_batch("batch-8x10k", [config_8b_10k(seed + 1000 * (i + 1)) for i in range(8)])
+
+
 CONFIGS: Dict[str, Callable[[], Workload]] = {
     "tiny": config_tiny,
     "8b-10k": config_8b_10k,

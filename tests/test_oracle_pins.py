@@ -407,3 +407,101 @@ def test_encoder_thresholds_monotone_and_extremes():
         prev_la, prev_ca = info["la_bits"], info["ca_bits"]
     # rows sum to one and the first row is the single cell p[0, 0] = 1
     assert np.allclose(info["p"].sum(axis=1), 1.0) and info["p"][0, 0] == 1.0
+
+
+# ---------------------------------------------------------------- several prompts in one call
+
+def _small_batch(gran=1, tile=64):
+    kw = dict(n_layers=1, n_q_heads=2, n_kv_heads=1, head_dim=64, tile=tile, cross_gran=gran)
+    a = wl.custom("ba", doc_lens=(130, 70, 200), query_len=40, p_loc=0.5, p_cross=0.3, seed=11, **kw)
+    b = wl.custom("bb", doc_lens=(), query_len=90, seed=12, **kw)                      # a prompt without documents
+    c = wl.custom("bc", doc_lens=(64, 333), query_len=1, p_loc=0.4, p_cross=0.5, seed=13, **kw)
+    return wl.make_batch("b3", [a, b, c])
+
+
+def test_batch_of_one_is_md_v1():
+    """PAPER.md:L267 (single-request TTFT) is the one-prompt case: MD-v1b of one prompt IS MD-v1."""
+    w = wl.custom("one", n_layers=2, n_q_heads=2, doc_lens=(100, 260, 64), query_len=70, tile=64, seed=5)
+    sh = w.shape
+    single = so.decode_metadata(sh.doc_offsets, sh.query_len, sh.tile, sh.cross_gran, sh.n_layers, sh.n_q_heads, w.la_vec, w.ca_vec)
+    b = wl.make_batch("one-b", [w])
+    batch = so.decode_metadata_batch(b.prompts, sh.tile, sh.cross_gran, sh.n_layers, sh.n_q_heads, b.la_vec, b.ca_vec)
+    for k in ("tile_base", "tile_seg", "tile_row0", "tile_rows", "cross_ptr", "local_cnt", "local_ptr"):
+        assert np.array_equal(single[k], batch[k]), k
+    assert batch["cross_cap"] == single["cross_cap"] and batch["local_cap"] == single["local_cap"]
+    for l in range(sh.n_layers):
+        for h in range(sh.n_q_heads):
+            nc, nl = int(single["cross_ptr"][l, h, -1]), int(single["local_ptr"][l, h, -1])
+            assert np.array_equal(single["cross_idx"][l, h, :nc], batch["cross_idx"][l, h, :nc])
+            assert np.array_equal(single["local_idx"][l, h, :nl], batch["local_idx"][l, h, :nl])
+    assert list(batch["seg_doc"]) == [0, 1, 2, -1] and list(batch["seg_first"]) == [0, 0, 0, 0]
+
+
+@pytest.mark.parametrize("gran", [1, 64])
+def test_batch_mask_is_block_diagonal_and_round_trips(gran):
+    """A row of prompt p sees keys of prompt p only, by the single-prompt rule (L147-149 per request); the MD-v1b
+    container, read back by its own rules, reproduces that mask (the round-trip pin of the container)."""
+    b = _small_batch(gran)
+    sh = b.head_shape
+    rows = list(range(0, b.n_tokens, 7)) + [int(x) for x in b.row_base[1:] - 1] + [int(x) for x in b.row_base[:-1]]
+    md = so.decode_metadata_batch(b.prompts, sh.tile, gran, 1, sh.n_q_heads, b.la_vec, b.ca_vec)
+    n_docs = len(b.doc_lens)
+    for h in range(sh.n_q_heads):
+        la = [b.la_vec(0, h, d) for d in range(n_docs)]
+        ca = [b.ca_vec(0, h, d) for d in range(n_docs)]
+        mask = so.expand_mask_rows_batch(b.prompts, sh.tile, gran, la, ca, rows)
+        for ri, q in enumerate(rows):
+            p = so.prompt_of_row(q, b.row_base)
+            lo, hi = int(b.row_base[p]), int(b.row_base[p + 1])
+            assert not mask[ri, :lo].any() and not mask[ri, hi:].any()
+            # inside its prompt the row is the single-prompt row
+            m = b.members[p]
+            la_p, ca_p = so.head_vectors(m, 0, h)
+            ref = so.expand_mask_rows(m.shape.doc_offsets, m.shape.query_len, sh.tile, gran, la_p, ca_p, [q - lo])
+            assert np.array_equal(mask[ri, lo:hi], ref[0])
+        back = so.metadata_batch_to_mask_rows(md, b.prompts, sh.tile, gran, 0, h, rows)
+        assert np.array_equal(back, mask)
+
+
+def test_batch_container_rules():
+    b = _small_batch()
+    sh = b.head_shape
+    md = so.decode_metadata_batch(b.prompts, sh.tile, 1, 1, sh.n_q_heads, b.la_vec, b.ca_vec)
+    assert list(md["seg_doc"]) == [0, 1, 2, -1, -1, 3, 4, -1]
+    assert list(md["seg_first"]) == [0, 0, 0, 0, 4, 5, 5, 5]
+    cp = md["cross_ptr"][0]
+    for h in range(sh.n_q_heads):
+        assert cp[h, 0] == 0 and cp[h, 3] % 128 == 0          # every prompt's cross list starts at a multiple of 128
+        assert np.all(np.diff(cp[h, :3]) >= 0) and np.all(np.diff(cp[h, 3:]) >= 0)
+        # counts inside a prompt are plain popcounts of its documents' valid CA bits
+        for d in (0, 1, 3):
+            bits = so.read_bits(b.ca_vec(0, h, d), so.ca_vector_bits(b.doc_lens[d], sh.tile, 1))
+            assert cp[h, d + 1] - cp[h, d] == int(bits.sum())
+        # a query tile lists the tiles of its own prompt, first to itself (L243, per request)
+        for p in range(3):
+            seg_q = int(np.nonzero(md["seg_first"] == md["seg_first"][[3, 4, 7][p]])[0][-1])
+            f = int(md["tile_base"][int(md["seg_first"][seg_q])])
+            for t in range(int(md["tile_base"][seg_q]), int(md["tile_base"][seg_q + 1])):
+                lo, hi = int(md["local_ptr"][0, h, t]), int(md["local_ptr"][0, h, t + 1])
+                assert list(md["local_idx"][0, h, lo:hi]) == list(range(f, t + 1))
+
+
+def test_batch_attention_rows_against_brute_force():
+    """Slicing check: a row of the packed batch, brute-forced in fp64 over the GLOBAL K/V with the keys the batch
+    mask allows, equals the oracle's per-prompt computation."""
+    b = _small_batch()
+    sh = b.head_shape
+    q, k, v = b.qkv(0)
+    n_docs = len(b.doc_lens)
+    rows = [5, 399, 439, 440, 529, 530, 600, 926, 927]
+    for h in range(sh.n_q_heads):
+        la = [b.la_vec(0, h, d) for d in range(n_docs)]
+        ca = [b.ca_vec(0, h, d) for d in range(n_docs)]
+        o, lse = so.sift_attention_rows_batch(q, k, v, h, b.prompts, sh.tile, 1, la, ca, rows, dtype=torch.float64)
+        mask = so.expand_mask_rows_batch(b.prompts, sh.tile, 1, la, ca, rows)
+        kvh = so.kv_head_of(h, sh.n_q_heads, sh.n_kv_heads)
+        for ri, r in enumerate(rows):
+            allowed = np.nonzero(mask[ri])[0]
+            ob, lb = so.brute_force_row(q[r, h].double().numpy(), k[:, kvh].double().numpy(), v[:, kvh].double().numpy(),
+                                        allowed, 1.0 / math.sqrt(sh.head_dim))
+            assert np.allclose(o[ri].numpy(), ob, atol=1e-9) and abs(float(lse[ri]) - lb) < 1e-9
