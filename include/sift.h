@@ -52,7 +52,18 @@ typedef struct {
   int32_t tile;       /* T: 64 or 128 (M-block = N-block = T) */
   int32_t cross_gran; /* G: 1 = one CA bit per key token (BASELINE.json configs); tile = one bit per page */
   const int32_t* doc_offsets; /* HOST, n_docs + 1 entries */
+  /* ---- several prompts in one call (optional; struct_size = SIFT_SHAPE_SIZE_V1 or n_prompts <= 1: one prompt) ----
+   * PAPER.md:L67 (TTFT gates decode batching), L267 (the paper itself measures one request at a time).
+   * The prompts are packed back to back on the token axis: prompt p = documents [prompt_doc_start[p],
+   * prompt_doc_start[p+1]) in order, then its query of prompt_query_len[p] rows; a row attends keys of its own prompt
+   * only.  doc_offsets stays the running sum of the DOCUMENT lengths over all n_docs documents (queries not counted);
+   * query_len is ignored; N = doc_offsets[n_docs] + sum of prompt_query_len.  A prompt may have no documents.
+   * n_docs + n_prompts <= SIFT_MAX_DOCS + 1.  la_doc_off / ca_doc_off are indexed by the document's index. */
+  int32_t n_prompts;
+  const int32_t* prompt_doc_start; /* HOST, n_prompts + 1 entries, [0] = 0, [n_prompts] = n_docs, non-decreasing */
+  const int32_t* prompt_query_len; /* HOST, n_prompts entries, >= 0 */
 } sift_shape;
+#define SIFT_SHAPE_SIZE_V1 ((uint32_t)offsetof(sift_shape, n_prompts)) /* the struct before the prompt fields */
 
 /* Byte offsets (from the start of the metadata buffer) of the arrays of container "MD-v1".
  * All arrays are int32.  Canonical arrays (compared bit-exactly with the oracle):
@@ -63,7 +74,12 @@ typedef struct {
  *                                  document d attend entries [0, cross_ptr[d])
  *   local_cnt [L][Hq][NT], local_ptr [L][Hq][NT+1], local_idx [L][Hq][local_cap]
  *                                  per M-block: ascending global tile ids of marked LA tiles; query M-block t: 0..t
- * Private arrays (scheduler): sched [L][n_items], counters [L][2]. */
+ * Several prompts ("MD-v1b"): segments (documents and queries) and documents are numbered in token order,
+ * tile_base has n_docs + n_prompts + 1 entries; the cross list of every prompt starts at a multiple of 128, so
+ * cross_ptr[d] is a running count that is rounded up at each prompt's first document, and document d of a prompt
+ * whose first document is d0 attends entries [cross_ptr[d0], cross_ptr[d]); query tile t of a prompt whose first tile
+ * is f lists f..t.  One prompt: exactly the arrays above.
+ * Private arrays: seg_info [n_seg][4], sched [L][n_items], counters [L][2], sort keys [L][n_items]. */
 typedef struct {
   uint32_t struct_size;
   int32_t n_tiles;   /* NT */
@@ -75,6 +91,9 @@ typedef struct {
   size_t cross_ptr, cross_idx, local_cnt, local_ptr, local_idx;
   size_t mblock_tile0, sched, counters;
   size_t total_bytes;
+  int32_t n_seg;     /* segments: n_docs + max(n_prompts, 1) */
+  int32_t n_tokens;  /* N */
+  size_t seg_info;   /* private: per segment {document index or -1, first document of its prompt, first row of its prompt, first tile of its prompt} */
 } sift_md_layout;
 
 const char* sift_version(void);

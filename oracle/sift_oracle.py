@@ -498,7 +498,7 @@ def decode_metadata_batch(prompts: Sequence[Prompt], tile: int, gran: int, n_lay
         lcap += sum(int(x) * (int(x) + 1) // 2 for x in m["P"][:npd])
         lcap += sum(t + 1 for t in range(int(m["tile_base"][npd]), int(m["NT"])))
     cross_ptr = np.zeros((n_layers, n_heads, n_docs + 1), np.int32)
-    cross_idx = np.full((n_layers, n_heads, max(ccap, 128)), -1, np.int32)
+    cross_idx = np.full((n_layers, n_heads, max(ccap, 1)), -1, np.int32)
     local_cnt = np.zeros((n_layers, n_heads, nt), np.int32)
     local_ptr = np.zeros((n_layers, n_heads, nt + 1), np.int32)
     local_idx = np.full((n_layers, n_heads, max(lcap, 1)), -1, np.int32)
@@ -532,7 +532,7 @@ def decode_metadata_batch(prompts: Sequence[Prompt], tile: int, gran: int, n_lay
             "tile_base": np.asarray(tile_base, np.int32), "NT": nt, "tile_seg": np.asarray(tile_seg, np.int32),
             "tile_row0": np.asarray(tile_row0, np.int32), "tile_rows": np.asarray(tile_rows, np.int32),
             "cross_ptr": cross_ptr, "cross_idx": cross_idx, "local_cnt": local_cnt, "local_ptr": local_ptr,
-            "local_idx": local_idx, "cross_cap": max(ccap, 128), "local_cap": max(lcap, 1)}
+            "local_idx": local_idx, "cross_cap": ccap, "local_cap": max(lcap, 1)}
 
 
 def metadata_batch_to_mask_rows(md: Dict[str, np.ndarray], prompts: Sequence[Prompt], tile: int, gran: int,

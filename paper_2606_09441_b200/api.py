@@ -24,7 +24,9 @@ class SiftShape(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_layers", C.c_int32), ("n_q_heads", C.c_int32),
                 ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32), ("n_docs", C.c_int32),
                 ("query_len", C.c_int32), ("tile", C.c_int32), ("cross_gran", C.c_int32),
-                ("doc_offsets", C.POINTER(C.c_int32))]
+                ("doc_offsets", C.POINTER(C.c_int32)),
+                ("n_prompts", C.c_int32), ("prompt_doc_start", C.POINTER(C.c_int32)),
+                ("prompt_query_len", C.POINTER(C.c_int32))]
 
 
 class SiftMdLayout(C.Structure):
@@ -32,7 +34,8 @@ class SiftMdLayout(C.Structure):
                 ("local_cap", C.c_int32), ("n_mblocks", C.c_int32), ("n_items", C.c_int32)] + \
                [(n, C.c_size_t) for n in ("tile_base", "tile_seg", "tile_row0", "tile_rows", "cross_ptr", "cross_idx",
                                           "local_cnt", "local_ptr", "local_idx", "mblock_tile0", "sched", "counters",
-                                          "total_bytes")]
+                                          "total_bytes")] + \
+               [("n_seg", C.c_int32), ("n_tokens", C.c_int32), ("seg_info", C.c_size_t)]
 
 
 class SiftError(RuntimeError):
@@ -103,20 +106,44 @@ class Shape:
     query_len: int
     tile: int
     cross_gran: int = 1
+    # several prompts in one call (sift.h): documents [prompt_doc_start[p], prompt_doc_start[p+1]) + a query each
+    prompt_doc_start: Optional[np.ndarray] = None
+    prompt_query_len: Optional[np.ndarray] = None
 
     def __post_init__(self):
         self.doc_offsets = np.ascontiguousarray(self.doc_offsets, dtype=np.int32)
+        ip = C.POINTER(C.c_int32)
+        n_prompts, pds, pql = 0, ip(), ip()
+        if self.prompt_doc_start is not None:
+            self.prompt_doc_start = np.ascontiguousarray(self.prompt_doc_start, dtype=np.int32)
+            self.prompt_query_len = np.ascontiguousarray(self.prompt_query_len, dtype=np.int32)
+            n_prompts = len(self.prompt_query_len)
+            pds, pql = self.prompt_doc_start.ctypes.data_as(ip), self.prompt_query_len.ctypes.data_as(ip)
         self._c = SiftShape(C.sizeof(SiftShape), self.n_layers, self.n_q_heads, self.n_kv_heads, self.head_dim,
                             len(self.doc_offsets) - 1, self.query_len, self.tile, self.cross_gran,
-                            self.doc_offsets.ctypes.data_as(C.POINTER(C.c_int32)))
+                            self.doc_offsets.ctypes.data_as(ip), n_prompts, pds, pql)
 
     @classmethod
     def from_prompt(cls, ps) -> "Shape":
         return cls(ps.n_layers, ps.n_q_heads, ps.n_kv_heads, ps.head_dim, ps.doc_offsets, ps.query_len, ps.tile,
                    ps.cross_gran)
 
+    @classmethod
+    def from_batch(cls, b) -> "Shape":
+        """b: workload.BatchWorkload (prompts packed back to back on the token axis)."""
+        if len(b.members) == 1:
+            return cls.from_prompt(b.members[0].shape)
+        hs = b.head_shape
+        off = np.concatenate([[0], np.cumsum(np.asarray(b.doc_lens, dtype=np.int64))])
+        return cls(hs.n_layers, hs.n_q_heads, hs.n_kv_heads, hs.head_dim, off, 0, hs.tile, hs.cross_gran,
+                   b.prompt_doc_start, b.prompt_query_len)
+
     @property
     def n_tokens(self) -> int:
+        if self.prompt_query_len is not None and len(self.prompt_query_len) > 1:
+            return int(self.doc_offsets[-1]) + int(self.prompt_query_len.sum())
+        if self.prompt_query_len is not None and len(self.prompt_query_len) == 1:
+            return int(self.doc_offsets[-1]) + int(self.prompt_query_len[0])
         return int(self.doc_offsets[-1]) + self.query_len
 
     @property
@@ -208,12 +235,12 @@ def metadata_views(shape: Shape, metadata: torch.Tensor) -> Dict[str, torch.Tens
         n = int(np.prod(dims))
         return m32[off // 4: off // 4 + n].view(*dims)
     return {
-        "tile_base": v(lay.tile_base, D + 2), "tile_seg": v(lay.tile_seg, NT), "tile_row0": v(lay.tile_row0, NT),
+        "tile_base": v(lay.tile_base, lay.n_seg + 1), "tile_seg": v(lay.tile_seg, NT), "tile_row0": v(lay.tile_row0, NT),
         "tile_rows": v(lay.tile_rows, NT), "cross_ptr": v(lay.cross_ptr, L, H, D + 1),
         "cross_idx": v(lay.cross_idx, L, H, lay.cross_cap), "local_cnt": v(lay.local_cnt, L, H, NT),
         "local_ptr": v(lay.local_ptr, L, H, NT + 1), "local_idx": v(lay.local_idx, L, H, lay.local_cap),
         "mblock_tile0": v(lay.mblock_tile0, lay.n_mblocks + 1), "sched": v(lay.sched, L, lay.n_items),
-        "counters": v(lay.counters, L, 2),
+        "counters": v(lay.counters, L, 2), "seg_info": v(lay.seg_info, lay.n_seg, 4),
     }
 
 

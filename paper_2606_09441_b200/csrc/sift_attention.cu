@@ -62,6 +62,7 @@ static_assert(kNQ * kRegsSoftmax + 2 * kRegsOther <= (kNumThreads / 128) * kRegs
 struct AttnParams {
   // metadata (null in dense mode)
   const int32_t *tile_seg, *tile_row0, *tile_rows, *mblock_tile0;
+  const int32_t* seg_info;   // [n_seg][4]: document index (-1: query), first document / first row / first tile of the prompt
   const int32_t *cross_ptr, *cross_idx, *local_cnt, *local_ptr, *local_idx;  // already offset to the layer
   const int32_t* sched;                                                      // already offset to the layer
   int32_t* counters;                                                         // [2]: next item, finished CTAs
@@ -108,7 +109,9 @@ struct Item {
   int is_dense;            // DENSE (query rows / comparator) or DOC
   int row0[kNQ], rows[kNQ];  // global first row and valid rows of each query tile (rows <= 0: tile absent)
   int tile_id[kNQ];
-  int cp;                  // DOC: number of cross entries of its document
+  int c0, cp;              // DOC: its document attends cross entries [c0, cp) of the head's list (c0 = start of the
+                           // prompt's list, a multiple of 128; 0 with one prompt)
+  int kbase;               // DENSE: first key row (first row of the prompt; 0 with one prompt and in the comparator)
   int lptr[kNQ], lcnt[kNQ];  // DOC: local list of each tile
 };
 
@@ -117,7 +120,7 @@ __device__ __forceinline__ Item load_item(const AttnParams& p, int code) {
   const int h = code >> 20, mb = code & 0xFFFFF;
   it.h = h;
   it.kvh = h / (p.n_q_heads / p.n_kv_heads);
-  it.cp = 0;
+  it.c0 = 0; it.cp = 0; it.kbase = 0;
   if (p.dense) {
     it.is_dense = 1;
 #pragma unroll
@@ -131,9 +134,14 @@ __device__ __forceinline__ Item load_item(const AttnParams& p, int code) {
   const int t0 = p.mblock_tile0[mb];
   const int nt = min(kNQ, p.mblock_tile0[mb + 1] - t0);
   const int seg = p.tile_seg[t0];
-  it.is_dense = (seg == p.n_docs);
+  const int4 si = reinterpret_cast<const int4*>(p.seg_info)[seg];
+  it.is_dense = (si.x < 0);
+  it.kbase = si.z;
   const int64_t lh = h;  // pointers are already offset to the layer
-  if (!it.is_dense) it.cp = p.cross_ptr[lh * (p.n_docs + 1) + seg];
+  if (!it.is_dense) {
+    it.c0 = p.cross_ptr[lh * (p.n_docs + 1) + si.y];
+    it.cp = p.cross_ptr[lh * (p.n_docs + 1) + si.x];
+  }
 #pragma unroll
   for (int q = 0; q < kNQ; ++q) {
     if (q < nt) {
@@ -329,23 +337,23 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       if (it.is_dense) {
         int n[kNQ], total = 0;
 #pragma unroll
-        for (int q = 0; q < kNQ; ++q) { n[q] = dense_steps(it.row0[q], it.rows[q]); total = max(total, n[q]); }
+        for (int q = 0; q < kNQ; ++q) { n[q] = dense_steps(it.row0[q] - it.kbase, it.rows[q]); total = max(total, n[q]); }
         for (int j = 0; j < total; ++j) {
           int act = 0;
 #pragma unroll
           for (int q = 0; q < kNQ; ++q) act |= (j < n[q]) << q;
-          emit(false, j * kBN, act, j == total - 1);
+          emit(false, it.kbase + j * kBN, act, j == total - 1);
         }
       } else {
         int present = 0, nloc = 0;
 #pragma unroll
         for (int q = 0; q < kNQ; ++q) { present |= (it.rows[q] > 0) << q; nloc += it.lcnt[q]; }
-        const int ngroups = p.paged ? 0 : (it.cp + kBN - 1) / kBN;
+        const int ngroups = p.paged ? 0 : (it.cp - it.c0 + kBN - 1) / kBN;
         if (p.paged) {                     // page-granular cross keys: the listed pages as tiled boxes
           const int32_t* cidx = p.cross_idx + (int64_t)it.h * p.cross_cap;
-          for (int e = 0; e < it.cp; ++e) emit(false, p.tile_row0[cidx[e]], present, e == it.cp - 1 && nloc == 0);
+          for (int e = it.c0; e < it.cp; ++e) emit(false, p.tile_row0[cidx[e]], present, e == it.cp - 1 && nloc == 0);
         }
-        for (int g = 0; g < ngroups; ++g) emit(true, g * kBN, present, g == ngroups - 1 && nloc == 0);
+        for (int g = 0; g < ngroups; ++g) emit(true, it.c0 + g * kBN, present, g == ngroups - 1 && nloc == 0);
         const int32_t* lidx = p.local_idx + (int64_t)it.h * p.local_cap;
         int pos[kNQ];
 #pragma unroll
@@ -388,7 +396,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       int has_steps;
       {
         const Item it = load_item(p, code);
-        bool hs = it.is_dense || it.cp > 0;
+        bool hs = it.is_dense || it.cp > it.c0;
 #pragma unroll
         for (int q = 0; q < kNQ; ++q) hs = hs || it.lcnt[q] > 0;
         has_steps = __shfl_sync(0xffffffffu, (int)hs, 0);
@@ -493,7 +501,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       const int code = info[1 + slot];
       mbar_arrive(bar(S::bItemEmpty + slot));
       if (code < 0) break;
-      int row0, rows, h, ngroups, nsteps, diag_step, lim;
+      int row0, rows, h, ngroups, nsteps, diag_step, lim, c0;
       bool paged_item;
       {
         const Item it = load_item(p, code);
@@ -501,21 +509,22 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         const int lcnt = q ? it.lcnt[1] : it.lcnt[0], lptr = q ? it.lptr[1] : it.lptr[0];
         const int tile_id = q ? it.tile_id[1] : it.tile_id[0];
         if (rows <= 0) continue;
-        ngroups = it.is_dense ? 0 : (p.paged ? it.cp : (it.cp + kBN - 1) / kBN);
-        nsteps = it.is_dense ? dense_steps(row0, rows) : ngroups + lcnt;
+        c0 = it.c0;
+        ngroups = it.is_dense ? 0 : (p.paged ? it.cp - it.c0 : (it.cp - it.c0 + kBN - 1) / kBN);
+        nsteps = it.is_dense ? dense_steps(row0 - it.kbase, rows) : ngroups + lcnt;
         diag_step = -1;                                   // the step (if any) that is the causally masked diagonal tile
         if (!it.is_dense && lcnt > 0 && p.local_idx[(int64_t)h * p.local_cap + lptr + lcnt - 1] == tile_id)
           diag_step = nsteps - 1;
         // columns [0, lim) of the current step are allowed for this row; lim drops by kBN per step in the cross
         // phase (ragged last group) and in DENSE items (causal frontier)
-        lim = it.is_dense ? row0 + r + 1 : it.cp;
+        lim = it.is_dense ? row0 - it.kbase + r + 1 : it.cp - it.c0;
         if (it.is_dense) ngroups = nsteps;                // "frontier" steps: all of them
         paged_item = p.paged && !it.is_dense;
       }
       float m = -INFINITY, l = 0.f;
       for (int e = 0; e < nsteps; ++e, lim -= kBN) {
         int cur_lim = (e < ngroups) ? lim : (e == diag_step ? min(tile_lim, r + 1) : tile_lim);
-        if (paged_item && e < ngroups) cur_lim = p.tile_rows[p.cross_idx[(int64_t)h * p.cross_cap + e]];   // a page may be ragged
+        if (paged_item && e < ngroups) cur_lim = p.tile_rows[p.cross_idx[(int64_t)h * p.cross_cap + c0 + e]];   // a page may be ragged
         mbar_wait(bar(S::bSFull + q), sph, 301);
         sph ^= 1;
         tc_fence_after();
@@ -711,6 +720,7 @@ extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, co
   const int64_t lh0 = (int64_t)layer * Hq;
   p.tile_seg = at(lay.tile_seg); p.tile_row0 = at(lay.tile_row0); p.tile_rows = at(lay.tile_rows);
   p.mblock_tile0 = at(lay.mblock_tile0);
+  p.seg_info = at(lay.seg_info);
   p.cross_ptr = at(lay.cross_ptr) + lh0 * (D + 1);
   p.cross_idx = at(lay.cross_idx) + lh0 * lay.cross_cap;
   p.local_cnt = at(lay.local_cnt) + lh0 * lay.n_tiles;
@@ -721,7 +731,7 @@ extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, co
   p.n_items = lay.n_items; p.n_docs = D; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap;
   p.local_cap = lay.local_cap; p.n_mblocks = lay.n_mblocks;
   p.dense = 0;
-  p.n_tokens = shape->doc_offsets[D] + shape->query_len;
+  p.n_tokens = lay.n_tokens;
   p.n_q_heads = Hq; p.n_kv_heads = shape->n_kv_heads; p.tile = shape->tile;
   p.paged = (shape->cross_gran != 1);
   p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;

@@ -16,15 +16,24 @@ namespace sift {
 
 // Passed by value as a kernel parameter (CUDA >= 12.1 allows 32 KB of parameters): the decode grid and
 // the tile tables depend on the document offsets, which the ABI hands over as HOST memory.
+// Segments = documents and queries in token order (one prompt: its documents, then the query; several prompts: one
+// after the other).
+constexpr int kMaxSeg = SIFT_MAX_DOCS + 1;
 struct DocTable {
+  int32_t n_seg;
   int32_t n_docs;
-  int32_t query_len;
+  int32_t n_prompts;
   int32_t tile;
   int32_t gran;
-  int32_t off[SIFT_MAX_DOCS + 1];
-  int64_t la_off[SIFT_MAX_DOCS];
+  int32_t off[kMaxSeg + 1];        // first row of segment s; off[n_seg] = N
+  int16_t doc[kMaxSeg];            // document index of segment s, -1 for a query segment
+  int16_t first[kMaxSeg];          // first segment of s's prompt
+  int64_t la_off[SIFT_MAX_DOCS];   // by document index
   int64_t ca_off[SIFT_MAX_DOCS];
 };
+// fills n_seg, n_docs, n_prompts, tile, gran, off, doc, first from a validated shape
+void build_segments(const sift_shape* s, DocTable* dt);
+int64_t shape_n_tokens(const sift_shape* s);
 
 int set_error(int code, const char* fmt, ...);
 int validate_shape(const sift_shape* s);

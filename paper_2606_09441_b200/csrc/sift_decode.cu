@@ -38,7 +38,7 @@ struct DecodeParams {
   const uint8_t* ca;
   int32_t *tile_base, *tile_seg, *tile_row0, *tile_rows;
   int32_t *cross_ptr, *cross_idx, *local_cnt, *local_ptr, *local_idx;
-  int32_t *mblock_tile0, *sched, *counters, *sched_key;
+  int32_t *mblock_tile0, *sched, *counters, *sched_key, *seg_info;
   int32_t n_q_heads, n_kv_heads, n_tiles, cross_cap, local_cap, n_mblocks, n_items, gran;
   int32_t kv_per_group;   // kv heads whose work items are scheduled together (sched_kv_heads_per_group)
   int32_t cross_parts;    // CTAs per (layer, head) for the cross list: 4 when the grid would not fill the GPU, else 1
@@ -170,46 +170,49 @@ __device__ __forceinline__ int msb_bit(const uint8_t* __restrict__ v, int n) {
 
 __global__ void __launch_bounds__(kDecodeThreads)
 sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
-  __shared__ int s_tile_base[SIFT_MAX_DOCS + 2];
-  __shared__ int s_wstart[SIFT_MAX_DOCS + 2];
-  __shared__ int s_mb_base[SIFT_MAX_DOCS + 2];
-  // per-document copies of the kernel-parameter table: a per-lane index into the constant bank is replayed once per
-  // distinct address, shared memory is not
-  __shared__ int s_off[SIFT_MAX_DOCS + 2];        // first row of the segment; s_off[D + 1] = n_tokens
-  __shared__ int s_ca_lead[SIFT_MAX_DOCS];        // bit offset of the head's CA vector inside its first covering word
-  __shared__ int64_t s_doc64[2 * SIFT_MAX_DOCS];  // (the scheduler reuses these 8 KB for its bucket cache)
+  // tables per segment (documents and queries in token order; index S = totals)
+  __shared__ int s_tile_base[kMaxSeg + 1];
+  __shared__ int s_wstart[kMaxSeg + 1];
+  __shared__ int s_mb_base[kMaxSeg + 1];
+  // copies of the kernel-parameter table: a per-lane index into the constant bank is replayed once per distinct
+  // address, shared memory is not
+  __shared__ int s_off[kMaxSeg + 1];              // first row of the segment; s_off[S] = n_tokens
+  __shared__ short s_sdoc[kMaxSeg], s_sfirst[kMaxSeg];   // document index (-1: query), first segment of the prompt
+  __shared__ int s_ca_lead[kMaxSeg];              // bit offset of the head's CA vector inside its first covering word
+  __shared__ int64_t s_doc64[2 * kMaxSeg];
   int64_t* s_ca_word = s_doc64;                   // index (in 32-bit words from the 4-byte aligned base of p.ca) of that word
-  int64_t* s_la_off = s_doc64 + SIFT_MAX_DOCS;
+  int64_t* s_la_off = s_doc64 + kMaxSeg;
+  __shared__ int s_pad[kMaxSeg + 1];              // several prompts: list offset added to the raw bit rank (see below)
   __shared__ int s_scan[kDecodeThreads / 32 + 1];
-  __shared__ int s_stage[kStageEntries + kStageEntries / 16];   // compacted entries of one 256-word chunk (denser chunks go straight to global)
+  __shared__ int s_stage[kStageEntries + kStageEntries / 16];   // warp-private staging slices | per-segment counts | histogram
   __shared__ int s_bscan[2][(kWPT > kTPT ? kWPT : kTPT) * (kDecodeThreads / 32)];
 
   const int tid = threadIdx.x;
   const int h = blockIdx.x, l = blockIdx.y;
-  const int D = dt.n_docs, T = dt.tile, G = dt.gran;
+  const int S = dt.n_seg, D = dt.n_docs, T = dt.tile, G = dt.gran;
   const int64_t lh = (int64_t)l * p.n_q_heads + h;
   constexpr int NQ = SIFT_Q_TILES_PER_ITEM;
 
   // ---- step 0: per-segment tables (tiles, covering words of this head's CA vectors, M-blocks) ----------
-  // One warp scans the D + 1 segments 32 at a time (three running sums through shuffles); the other warps wait at a
+  // One warp scans the segments 32 at a time (three running sums through shuffles); the other warps wait at a
   // single barrier.  (The first version ran three block-wide scans per 256 segments in every CTA.)
   const int tsh = p.tile_shift, gsh = p.gran_shift;
   if (tid < 32) {
     int carry_t = 0, carry_w = 0, carry_m = 0;
-    for (int d0 = 0; d0 <= D; d0 += 32) {
+    for (int d0 = 0; d0 < S; d0 += 32) {
       const int d = d0 + tid;
       int pd = 0, nw = 0;
-      if (d < D) {
-        const int o0 = dt.off[d], len = dt.off[d + 1] - o0;
+      if (d < S) {
+        const int o0 = dt.off[d], len = dt.off[d + 1] - o0, dc = dt.doc[d];
         pd = (len + T - 1) >> tsh;
-        const int nbits = (len + G - 1) >> gsh;
-        const uint64_t a = (reinterpret_cast<uintptr_t>(p.ca) & 3) + (uint64_t)(dt.ca_off[d] + lh * ((nbits + 7) >> 3));
-        const int lead = (int)(a & 3);
-        nw = (lead * 8 + nbits + 31) >> 5;
-        s_off[d] = o0; s_ca_lead[d] = lead * 8; s_ca_word[d] = (int64_t)(a >> 2); s_la_off[d] = dt.la_off[d];
-      } else if (d == D) {
-        pd = (dt.query_len + T - 1) >> tsh;
-        s_off[D] = dt.off[D]; s_off[D + 1] = dt.off[D] + dt.query_len;
+        s_off[d] = o0; s_sdoc[d] = (short)dc; s_sfirst[d] = dt.first[d];
+        if (dc >= 0) {
+          const int nbits = (len + G - 1) >> gsh;
+          const uint64_t a = (reinterpret_cast<uintptr_t>(p.ca) & 3) + (uint64_t)(dt.ca_off[dc] + lh * ((nbits + 7) >> 3));
+          const int lead = (int)(a & 3);
+          nw = (lead * 8 + nbits + 31) >> 5;
+          s_ca_lead[d] = lead * 8; s_ca_word[d] = (int64_t)(a >> 2); s_la_off[d] = dt.la_off[dc];
+        }
       }
       int it = pd, iw = nw, im = (pd + NQ - 1) / NQ;
 #pragma unroll
@@ -218,7 +221,7 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
                   c = __shfl_up_sync(0xffffffffu, im, o);
         if (tid >= o) { it += a; iw += b; im += c; }
       }
-      if (d <= D) {
+      if (d < S) {
         s_tile_base[d] = carry_t + it - pd;
         s_wstart[d] = carry_w + iw - nw;
         s_mb_base[d] = carry_m + im - (pd + NQ - 1) / NQ;
@@ -228,13 +231,14 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
       carry_m += __shfl_sync(0xffffffffu, im, 31);
     }
     if (tid == 0) {
-      s_tile_base[D + 1] = carry_t;
-      s_wstart[D + 1] = carry_w;   // s_wstart[D] == carry_w as well (the query has no CA words)
-      s_mb_base[D + 1] = carry_m;
+      s_tile_base[S] = carry_t;
+      s_wstart[S] = carry_w;
+      s_mb_base[S] = carry_m;
+      s_off[S] = dt.off[S];
     }
   }
   __syncthreads();
-  const int NT = s_tile_base[D + 1];
+  const int NT = s_tile_base[S];
   // blockIdx.z splits a (layer, head): z < kCrossParts = one range of the cross list, z = kCrossParts = the local lists
   // (and, for the first head, the tile tables).  Shortens the latency chain of a CTA (a single layer is latency-bound).
   const int kCrossParts = p.cross_parts;
@@ -245,13 +249,15 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
   const bool do_keys = p.split_keys ? ((int)blockIdx.z == kCrossParts + 1) : do_local;
   const bool writer = (h == 0 && l == 0 && do_local);
   if (writer) {
-    for (int d = tid; d <= D + 1; d += kDecodeThreads) p.tile_base[d] = s_tile_base[d];
-    for (int d = tid; d <= D; d += kDecodeThreads) {
+    for (int d = tid; d <= S; d += kDecodeThreads) p.tile_base[d] = s_tile_base[d];
+    for (int d = tid; d < S; d += kDecodeThreads) {
       const int pd = s_tile_base[d + 1] - s_tile_base[d];
       const int nb = (pd + NQ - 1) / NQ;
       for (int k = 0; k < nb; ++k) p.mblock_tile0[s_mb_base[d] + k] = s_tile_base[d] + k * NQ;
+      const int f = s_sfirst[d];
+      reinterpret_cast<int4*>(p.seg_info)[d] = make_int4(s_sdoc[d], s_sdoc[f], s_off[f], s_tile_base[f]);
     }
-    if (tid == 0) p.mblock_tile0[s_mb_base[D + 1]] = NT;
+    if (tid == 0) p.mblock_tile0[s_mb_base[S]] = NT;
   }
 
   // ---- cross list: CA bits of all documents, one virtual word sequence ---------------------------------
@@ -260,12 +266,12 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
   // same two barriers) turns the counts into offsets.
   int32_t* cross_ptr = p.cross_ptr + lh * (D + 1);
   int32_t* cross_idx = p.cross_idx + lh * p.cross_cap;
-  // masked stream-order bits of word v of the head's virtual word sequence, the global coordinate of its bit 0 and
-  // the document it closes (or -1)
-  const int top_d = upper_seg_top(D), top_d1 = upper_seg_top(D + 1);
+  // masked stream-order bits of word v of the head's virtual word sequence, the global coordinate of its bit 0, the
+  // segment it closes (or -1) and its segment
+  const int top_s = upper_seg_top(S);
   const uint32_t* ca_words = reinterpret_cast<const uint32_t*>(reinterpret_cast<uintptr_t>(p.ca) & ~(uintptr_t)3);
-  auto load_word = [&](int v, int& key0, int& closes, int* doc = nullptr) -> uint32_t {
-    const int d = upper_seg(s_wstart, D, v, top_d);
+  auto load_word = [&](int v, int& key0, int& closes, int* seg = nullptr) -> uint32_t {
+    const int d = upper_seg(s_wstart, S, v, top_s);   // (segments without words share a start: the last one owns it)
     const int wi = v - s_wstart[d];
     const int len = s_off[d + 1] - s_off[d];
     const int nbits = (len + G - 1) >> gsh;
@@ -280,13 +286,74 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
     // global coordinate of stream bit 0 of this word: key row (G == 1) or tile id (G == tile; a page is a tile)
     key0 = (G == 1 ? s_off[d] : s_tile_base[d]) + wi * 32 - lead;
     closes = (v + 1 == s_wstart[d + 1]) ? d : -1;
-    if (doc) *doc = d;
+    if (seg) *seg = d;
     return x & m;
+  };
+  const int all_words = s_wstart[S];
+  // marked bits per segment, as an exclusive prefix in s_stage[0 .. S] (s_stage[s] = marked bits before segment s)
+  auto count_segments = [&]() {
+    int* s_ccnt = s_stage;
+    for (int d = tid; d <= S; d += kDecodeThreads) s_ccnt[d] = 0;
+    __syncthreads();
+#pragma unroll 4
+    for (int v = tid; v < all_words; v += kDecodeThreads) {
+      int k0, cl, d;
+      const int c = __popc(load_word(v, k0, cl, &d));
+      if (c) atomicAdd(&s_ccnt[d + 1], c);
+    }
+    __syncthreads();
+    if (tid < 32) {
+      int carry = 0;
+      for (int d0 = 0; d0 <= S; d0 += 32) {
+        const int d = d0 + tid;
+        int v = (d <= S) ? s_ccnt[d] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int n = __shfl_up_sync(0xffffffffu, v, o);
+          if (tid >= o) v += n;
+        }
+        if (d <= S) s_ccnt[d] = carry + v;
+        carry += __shfl_sync(0xffffffffu, v, 31);
+      }
+    }
+    __syncthreads();
+  };
+  // Several prompts (MD-v1b): the list of every prompt starts at a multiple of 128 (the attention kernel reads whole
+  // groups of 128 entries), so an entry's position is its rank among the head's marked bits plus s_pad[its segment].
+  // s_pad[S] doubles as "several prompts".  One prompt: all zero, nothing to count.
+  const bool multi = dt.n_prompts > 1;
+  if (multi && do_cross) {
+    count_segments();
+    if (tid == 0) {
+      int pad = 0;
+      for (int sg = 0; sg < S; ++sg) {
+        if (s_sfirst[sg] == sg) pad = ((s_stage[sg] + pad + 127) & ~127) - s_stage[sg];
+        s_pad[sg] = pad;
+      }
+    }
+    __syncthreads();
+    // the tail of every prompt's list up to the next multiple of 128 must hold valid rows (gathered, then masked)
+    if ((int)blockIdx.z == kCrossParts - 1) {
+      for (int sg = 0; sg < S; ++sg) {
+        if (s_sdoc[sg] >= 0) continue;                      // at a query segment: its prompt's documents are counted
+        const int end = s_stage[sg] + s_pad[sg];
+        for (int i = end + tid; i < ((end + 127) & ~127); i += kDecodeThreads) cross_idx[i] = 0;
+      }
+    }
+    __syncthreads();                                        // (s_stage becomes the staging buffer)
+  } else {
+    for (int sg = tid; sg <= S; sg += kDecodeThreads) s_pad[sg] = 0;
+    __syncthreads();
+  }
+  // list offset of the document that follows segment sg (= the end of sg's own entries; rounded up if a new prompt starts)
+  auto next_doc_pad = [&](int sg) {
+    int n = sg + 1;
+    while (n < S && s_sdoc[n] < 0) ++n;
+    return n < S ? s_pad[n] : s_pad[sg];
   };
   // The word sequence of a head is cut into kCrossParts ranges, one CTA each (grid z): a CTA first popcounts the words
   // before its range (the bit vectors of a head are a few KB: re-reading them costs less than waiting for a prefix
   // from another CTA), which gives it the list offset of its first entry.
-  const int all_words = s_wstart[D];
   const int per = (all_words + kCrossParts - 1) / kCrossParts;
   const int w_lo = do_cross ? min(all_words, (int)blockIdx.z * per) : 0;
   const int total_words = do_cross ? min(all_words, w_lo + per) : 0;      // end of this CTA's range
@@ -303,12 +370,16 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
   int scan_no = 0;   // the two scan buffers alternate over ALL scans of the kernel (no trailing barrier needed)
   for (int base = w_lo; base < total_words; base += kWPT * kDecodeThreads) {
     uint32_t bits[kWPT];
-    int key0[kWPT], cnt[kWPT], dd[kWPT];
+    int key0[kWPT], cnt[kWPT], dd[kWPT], pad[kWPT];
 #pragma unroll
     for (int k = 0; k < kWPT; ++k) {
       const int v = base + k * kDecodeThreads + tid;
-      bits[k] = 0; key0[k] = 0; dd[k] = -1;
-      if (v < total_words) bits[k] = load_word(v, key0[k], dd[k]);
+      bits[k] = 0; key0[k] = 0; dd[k] = -1; pad[k] = 0;
+      if (v < total_words) {
+        int sg;
+        bits[k] = load_word(v, key0[k], dd[k], &sg);
+        pad[k] = s_pad[sg];
+      }
     }
 #pragma unroll
     for (int k = 0; k < kWPT; ++k) cnt[k] = __popc(bits[k]);                     // pass 1: count
@@ -320,15 +391,18 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
     // 4-byte stores (32 sectors per store instruction when the ffs loop wrote straight to global memory).
 #pragma unroll
     for (int k = 0; k < kWPT; ++k) {
-      if (dd[k] >= 0) cross_ptr[dd[k] + 1] = running + ex[k] + cnt[k];
+      if (dd[k] >= 0) cross_ptr[s_sdoc[dd[k]] + 1] = running + ex[k] + cnt[k] + next_doc_pad(dd[k]);
       const int lane = tid & 31, wid = tid >> 5;
       const int wbase = __shfl_sync(0xffffffffu, ex[k], 0);                      // list offset of the warp's first entry
       const int wtot = __shfl_sync(0xffffffffu, ex[k] + cnt[k], 31) - wbase;     // entries of the warp's 32 words
       if (wtot == 0) continue;                                                   // warp-uniform
+      // (a warp whose words straddle two prompts has two different pads: it writes straight to global memory)
+      const int pmin = __reduce_min_sync(0xffffffffu, cnt[k] ? pad[k] : 0x7fffffff);
+      const int pmax = __reduce_max_sync(0xffffffffu, cnt[k] ? pad[k] : -1);
       int32_t* dst = cross_idx + running + wbase;
       int o = ex[k] - wbase;
       uint32_t bk = bits[k];
-      if (wtot <= kWarpStage) {
+      if (wtot <= kWarpStage && pmin == pmax) {
         int* stage = s_stage + wid * kWarpStage;
         while (bk) {
           const int sb = __ffs(bk) - 1;
@@ -336,9 +410,11 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
           stage[o++] = key0[k] + sb;
         }
         __syncwarp();
+        dst += pmin;
         for (int i = lane; i < wtot; i += 32) dst[i] = stage[i];
         __syncwarp();
-      } else {                                            // more than half of the warp's 1024 bits set
+      } else {                                            // more than half of the warp's 1024 bits set, or two prompts
+        dst += pad[k];
         while (bk) {
           const int sb = __ffs(bk) - 1;
           bk &= bk - 1;
@@ -348,16 +424,15 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
     }
     running += pass_total;
   }
-  // entries in [total, roundup128(total)) must be valid rows: the attention kernel gathers whole groups
   if (do_cross) {
-    if (blockIdx.z == kCrossParts - 1)
+    // entries in [total, roundup128(total)) must be valid rows: the attention kernel gathers whole groups
+    if (!multi && (int)blockIdx.z == kCrossParts - 1)
       for (int i = running + tid; i < ((running + 127) & ~127); i += kDecodeThreads) cross_idx[i] = 0;
   } else if (do_local) {
     // ---- local lists: LA row popcounts, offsets, fill -------------------------------------------------
     int32_t* local_cnt = p.local_cnt + lh * NT;
     int32_t* local_ptr = p.local_ptr + lh * (NT + 1);
     int32_t* local_idx = p.local_idx + lh * p.local_cap;
-    const int tq0 = s_tile_base[D];          // first tile of the user query
     running = 0;
     for (int base = 0; base < NT; base += kTPT * kDecodeThreads) {
       int cnt[kTPT], dd[kTPT], ii[kTPT];
@@ -367,7 +442,7 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
         const int t = base + k * kDecodeThreads + tid;
         cnt[k] = 0; dd[k] = 0; ii[k] = 0; lv[k] = nullptr;
         if (t < NT) {
-          const int d = upper_seg(s_tile_base, D + 1, t, top_d1);
+          const int d = upper_seg(s_tile_base, S, t, top_s);
           const int i = t - s_tile_base[d];
           dd[k] = d; ii[k] = i;
           const int seg_len = s_off[d + 1] - s_off[d];
@@ -376,8 +451,8 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
             p.tile_row0[t] = s_off[d] + i * T;
             p.tile_rows[t] = min(T, seg_len - i * T);
           }
-          if (d == D) {
-            cnt[k] = t + 1;                                             // query M-block: all causal N-blocks (L243)
+          if (s_sdoc[d] < 0) {
+            cnt[k] = t - s_tile_base[s_sfirst[d]] + 1;                  // query M-block: all causal N-blocks of its prompt (L243)
           } else {
             const int pd = s_tile_base[d + 1] - s_tile_base[d];
             const int nbytes = (pd * (pd + 1) / 2 + 7) >> 3;
@@ -395,21 +470,21 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
           const int w0 = running + ex[k];
           local_cnt[t] = cnt[k];
           local_ptr[t] = w0;
-          if (t == tq0) s_scan[0] = w0;      // where the query tiles' lists start (filled by the whole block below)
-          if (dd[k] < D) la_row_fill(lv[k], ii[k], s_tile_base[dd[k]], local_idx + w0);
+          if (s_sdoc[dd[k]] >= 0) la_row_fill(lv[k], ii[k], s_tile_base[dd[k]], local_idx + w0);
         }
       }
       running += pass_total;
     }
     if (tid == 0) local_ptr[NT] = running;
     __syncthreads();
-    // query tile t lists all causal tiles 0 .. t: written by the whole block with coalesced stores (one thread per
-    // tile wrote up to ~500 entries one after the other in the first version)
-    {
-      int w0 = s_scan[0];
-      for (int t = tq0; t < NT; ++t) {
-        for (int j = tid; j <= t; j += kDecodeThreads) local_idx[w0 + j] = j;
-        w0 += t + 1;
+    // query tile t lists the tiles f .. t of its prompt: written by the whole block with coalesced stores (one thread
+    // per tile wrote up to ~500 entries one after the other in the first version)
+    for (int sg = 0; sg < S; ++sg) {
+      if (s_sdoc[sg] >= 0) continue;
+      const int f = s_tile_base[s_sfirst[sg]];
+      for (int t = s_tile_base[sg]; t < s_tile_base[sg + 1]; ++t) {
+        const int w0 = __ldcg(local_ptr + t);              // (written above by this block)
+        for (int j = tid; j <= t - f; j += kDecodeThreads) local_idx[w0 + j] = f + j;
       }
     }
   }
@@ -420,55 +495,32 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
     // of 128 gathered rows (G == 1) or one page per step (G == tile) + local tiles | dense steps of query tiles.
     // The counts are recounted here from the bits (a few KB, read by the list CTAs at the same time) instead of waiting
     // for the lists: every CTA of the layer only publishes, and the CTA that finishes last just sorts the keys.
-    {
-      __syncthreads();                                         // (the local lists above are done with s_stage / s_scan)
-      int* s_ccnt = s_stage;                                   // [D + 1]: entries in documents < d
-      for (int d = tid; d <= D; d += kDecodeThreads) s_ccnt[d] = 0;
-      __syncthreads();
-#pragma unroll 4
-      for (int v = tid; v < all_words; v += kDecodeThreads) {
-        int k0, cl, d;
-        const int c = __popc(load_word(v, k0, cl, &d));
-        if (c) atomicAdd(&s_ccnt[d + 1], c);
+    __syncthreads();                                         // (the local lists above are done with s_stage / s_scan)
+    count_segments();
+    const int* s_ccnt = s_stage;
+    const int groups = (p.n_kv_heads + p.kv_per_group - 1) / p.kv_per_group, bpg = kCostBuckets / groups;
+    const int g = h / ((p.n_q_heads / p.n_kv_heads) * p.kv_per_group);
+    int32_t* key = p.sched_key + (int64_t)l * p.n_items + (int64_t)h * p.n_mblocks;
+    static_assert(NQ == 2, "cost of an M-block: two tiles");
+    for (int mb = tid; mb < p.n_mblocks; mb += kDecodeThreads) {
+      const int seg = upper_seg(s_mb_base, S, mb, top_s);
+      const int t0 = s_tile_base[seg] + (mb - s_mb_base[seg]) * NQ;
+      const bool two = t0 + 1 < s_tile_base[seg + 1];
+      const int f = s_sfirst[seg];
+      int c;
+      if (s_sdoc[seg] >= 0) {
+        const int cp = s_ccnt[seg] - s_ccnt[f];              // marked keys of the prompt's earlier documents
+        const int cross_steps = (G == 1) ? (cp + 127) >> 7 : cp;
+        const int pd = s_tile_base[seg + 1] - s_tile_base[seg], i0 = t0 - s_tile_base[seg];
+        const uint8_t* lv = p.la + s_la_off[seg] + lh * ((pd * (pd + 1) / 2 + 7) >> 3);
+        c = (two ? 2 : 1) * cross_steps + la_row_count(lv, i0) + (two ? la_row_count(lv, i0 + 1) : 0);
+      } else {
+        // dense steps of the query tiles: keys from the prompt's first row to the tile's last row
+        const int r0 = s_off[seg] - s_off[f] + (t0 - s_tile_base[seg]) * T, rend = s_off[seg + 1] - s_off[f];
+        c = (min(r0 + T, rend) + 127) >> 7;
+        if (two) c += (min(r0 + 2 * T, rend) + 127) >> 7;
       }
-      __syncthreads();
-      if (tid < 32) {
-        int carry = 0;
-        for (int d0 = 0; d0 <= D; d0 += 32) {
-          const int d = d0 + tid;
-          int v = (d <= D) ? s_ccnt[d] : 0;
-#pragma unroll
-          for (int o = 1; o < 32; o <<= 1) {
-            const int n = __shfl_up_sync(0xffffffffu, v, o);
-            if (tid >= o) v += n;
-          }
-          if (d <= D) s_ccnt[d] = carry + v;
-          carry += __shfl_sync(0xffffffffu, v, 31);
-        }
-      }
-      __syncthreads();
-      const int groups = (p.n_kv_heads + p.kv_per_group - 1) / p.kv_per_group, bpg = kCostBuckets / groups;
-      const int g = h / ((p.n_q_heads / p.n_kv_heads) * p.kv_per_group);
-      int32_t* key = p.sched_key + (int64_t)l * p.n_items + (int64_t)h * p.n_mblocks;
-      static_assert(NQ == 2, "cost of an M-block: two tiles");
-      for (int mb = tid; mb < p.n_mblocks; mb += kDecodeThreads) {
-        const int seg = upper_seg(s_mb_base, D + 1, mb, top_d1);
-        const int t0 = s_tile_base[seg] + (mb - s_mb_base[seg]) * NQ;
-        const bool two = t0 + 1 < s_tile_base[seg + 1];
-        int c;
-        if (seg < D) {
-          const int cp = s_ccnt[seg];
-          const int cross_steps = (G == 1) ? (cp + 127) >> 7 : cp;
-          const int pd = s_tile_base[seg + 1] - s_tile_base[seg], i0 = t0 - s_tile_base[seg];
-          const uint8_t* lv = p.la + s_la_off[seg] + lh * ((pd * (pd + 1) / 2 + 7) >> 3);
-          c = (two ? 2 : 1) * cross_steps + la_row_count(lv, i0) + (two ? la_row_count(lv, i0 + 1) : 0);
-        } else {
-          const int r0 = s_off[D] + (t0 - s_tile_base[D]) * T;     // dense steps of the query tiles: keys 0 .. last row
-          c = (min(r0 + T, s_off[D + 1]) + 127) >> 7;
-          if (two) c += (min(r0 + 2 * T, s_off[D + 1]) + 127) >> 7;
-        }
-        key[mb] = g * bpg + (bpg - 1 - min(c, bpg - 1));
-      }
+      key[mb] = g * bpg + (bpg - 1 - min(c, bpg - 1));
     }
   }
 
@@ -539,6 +591,7 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   p.local_cnt = at(lay.local_cnt); p.local_ptr = at(lay.local_ptr); p.local_idx = at(lay.local_idx);
   p.mblock_tile0 = at(lay.mblock_tile0); p.sched = at(lay.sched); p.counters = at(lay.counters);
   p.sched_key = at(sched_key_offset(lay, s->n_layers));
+  p.seg_info = at(lay.seg_info);
   p.n_q_heads = s->n_q_heads; p.n_kv_heads = s->n_kv_heads; p.n_tiles = lay.n_tiles; p.cross_cap = lay.cross_cap; p.local_cap = lay.local_cap;
   p.n_mblocks = lay.n_mblocks; p.n_items = lay.n_items; p.gran = s->cross_gran;
   // few (layer, head) pairs (one layer of an 8B-class model = 32): the call is latency-bound, cut each head's cross list
@@ -547,7 +600,7 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   if (int rc = device_sm_count(&num_sms)) return rc;
   p.cross_parts = ((int64_t)s->n_q_heads * s->n_layers <= num_sms) ? kMaxCrossParts : 1;
   p.split_keys = (p.cross_parts > 1);
-  p.kv_per_group = sched_kv_heads_per_group((int64_t)s->doc_offsets[s->n_docs] + s->query_len, s->head_dim, s->n_kv_heads);
+  p.kv_per_group = sched_kv_heads_per_group(lay.n_tokens, s->head_dim, s->n_kv_heads);
   p.tile_shift = (s->tile == 128) ? 7 : 6;
   p.gran_shift = (s->cross_gran == 1) ? 0 : p.tile_shift;
   if (s->n_layers > kDoneRing / 4) return set_error(SIFT_ERR_UNSUPPORTED, "too many layers in one decode call");

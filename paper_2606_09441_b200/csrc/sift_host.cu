@@ -19,10 +19,21 @@ int set_error(int code, const char* fmt, ...) {
 
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+static int shape_n_prompts(const sift_shape* s) {
+  return (s->struct_size == sizeof(sift_shape) && s->n_prompts > 1) ? s->n_prompts : 1;
+}
+int64_t shape_n_tokens(const sift_shape* s) {
+  int64_t n = s->doc_offsets[s->n_docs];
+  const int np = shape_n_prompts(s);
+  if (np > 1) { for (int p = 0; p < np; ++p) n += s->prompt_query_len[p]; } else n += s->query_len;
+  return n;
+}
+
 int validate_shape(const sift_shape* s) {
   if (!s) return set_error(SIFT_ERR_INVALID_ARG, "shape is NULL");
-  if (s->struct_size != sizeof(sift_shape))
-    return set_error(SIFT_ERR_INVALID_ARG, "shape.struct_size %u != %zu", s->struct_size, sizeof(sift_shape));
+  if (s->struct_size != sizeof(sift_shape) && s->struct_size != SIFT_SHAPE_SIZE_V1)
+    return set_error(SIFT_ERR_INVALID_ARG, "shape.struct_size %u: expected %zu (or %u, the struct without the prompt fields)",
+                     s->struct_size, sizeof(sift_shape), SIFT_SHAPE_SIZE_V1);
   if (!s->doc_offsets) return set_error(SIFT_ERR_INVALID_ARG, "shape.doc_offsets is NULL");
   if (s->n_layers < 1 || s->n_q_heads < 1 || s->n_kv_heads < 1 || s->n_docs < 0 || s->query_len < 0)
     return set_error(SIFT_ERR_INVALID_ARG, "negative or zero dimension");
@@ -39,9 +50,42 @@ int validate_shape(const sift_shape* s) {
   for (int d = 0; d < s->n_docs; ++d)
     if (s->doc_offsets[d + 1] <= s->doc_offsets[d])
       return set_error(SIFT_ERR_INVALID_ARG, "doc_offsets not strictly increasing at %d", d);
-  int64_t n = (int64_t)s->doc_offsets[s->n_docs] + s->query_len;
-  if (n < 1 || n > (1 << 20)) return set_error(SIFT_ERR_UNSUPPORTED, "prompt of %lld rows (1 .. 2^20 supported)", (long long)n);
+  const int np = shape_n_prompts(s);
+  if (np > 1) {
+    if (!s->prompt_doc_start || !s->prompt_query_len)
+      return set_error(SIFT_ERR_INVALID_ARG, "n_prompts %d but prompt_doc_start / prompt_query_len is NULL", np);
+    if (s->n_docs + np > SIFT_MAX_DOCS + 1)
+      return set_error(SIFT_ERR_UNSUPPORTED, "n_docs + n_prompts = %d > %d", s->n_docs + np, SIFT_MAX_DOCS + 1);
+    if (s->prompt_doc_start[0] != 0 || s->prompt_doc_start[np] != s->n_docs)
+      return set_error(SIFT_ERR_INVALID_ARG, "prompt_doc_start must run from 0 to n_docs");
+    for (int p = 0; p < np; ++p)
+      if (s->prompt_doc_start[p + 1] < s->prompt_doc_start[p] || s->prompt_query_len[p] < 0)
+        return set_error(SIFT_ERR_INVALID_ARG, "prompt %d: decreasing prompt_doc_start or negative query length", p);
+  }
+  int64_t n = shape_n_tokens(s);
+  if (n < 1 || n > (1 << 20)) return set_error(SIFT_ERR_UNSUPPORTED, "prompt(s) of %lld rows (1 .. 2^20 supported)", (long long)n);
   return SIFT_OK;
+}
+
+void build_segments(const sift_shape* s, DocTable* dt) {
+  const int np = shape_n_prompts(s);
+  dt->n_docs = s->n_docs; dt->n_prompts = np; dt->tile = s->tile; dt->gran = s->cross_gran;
+  int seg = 0, row = 0;
+  for (int p = 0; p < np; ++p) {
+    const int d0 = np > 1 ? s->prompt_doc_start[p] : 0, d1 = np > 1 ? s->prompt_doc_start[p + 1] : s->n_docs;
+    const int qlen = np > 1 ? s->prompt_query_len[p] : s->query_len;
+    const int first = seg;
+    for (int d = d0; d < d1; ++d) {
+      dt->off[seg] = row; dt->doc[seg] = (int16_t)d; dt->first[seg] = (int16_t)first;
+      row += s->doc_offsets[d + 1] - s->doc_offsets[d];
+      ++seg;
+    }
+    dt->off[seg] = row; dt->doc[seg] = -1; dt->first[seg] = (int16_t)first;
+    row += qlen;
+    ++seg;
+  }
+  dt->off[seg] = row;
+  dt->n_seg = seg;
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -115,19 +159,24 @@ int compute_layout(const sift_shape* s, sift_md_layout* out) {
   int rc = validate_shape(s);
   if (rc) return rc;
   const int T = s->tile, D = s->n_docs, NQ = SIFT_Q_TILES_PER_ITEM;
-  int64_t nt = 0, lcap = 0, nmb = 0, ncross = 0;
-  for (int d = 0; d < D; ++d) {
-    int64_t p = ceil_div_i(s->doc_offsets[d + 1] - s->doc_offsets[d], T);
-    ncross += ceil_div_i(s->doc_offsets[d + 1] - s->doc_offsets[d], s->cross_gran);
+  static thread_local DocTable dt;
+  build_segments(s, &dt);
+  int64_t nt = 0, lcap = 0, nmb = 0, ccap = 0;
+  int64_t ncross = 0, first_tile = 0;       // of the current prompt
+  for (int sg = 0; sg < dt.n_seg; ++sg) {
+    const int64_t len = dt.off[sg + 1] - dt.off[sg];
+    const int64_t p = (len + T - 1) / T;
+    if (dt.first[sg] == sg) { first_tile = nt; ncross = 0; }
+    if (dt.doc[sg] >= 0) {
+      ncross += (len + s->cross_gran - 1) / s->cross_gran;
+      lcap += p * (p + 1) / 2;
+    } else {
+      for (int64_t t = nt; t < nt + p; ++t) lcap += t - first_tile + 1;   // a query tile lists its prompt's tiles up to itself
+      ccap += (ncross + 127) / 128 * 128;   // one entry per CA bit at most; every prompt's list in whole gather groups
+    }
     nt += p;
-    lcap += p * (p + 1) / 2;
     nmb += (p + NQ - 1) / NQ;
   }
-  int64_t pq = ceil_div_i(s->query_len, T);
-  for (int64_t t = nt; t < nt + pq; ++t) lcap += t + 1;
-  nt += pq;
-  nmb += (pq + NQ - 1) / NQ;
-  int64_t ccap = (ncross + 127) / 128 * 128;   // one entry per CA bit at most, rounded up to whole gather groups
   if (lcap >= (1ll << 31) || ccap >= (1ll << 31)) return set_error(SIFT_ERR_UNSUPPORTED, "index capacity >= 2^31");
   if (lcap < 1) lcap = 1;
   const int64_t LH = (int64_t)s->n_layers * s->n_q_heads;
@@ -140,7 +189,7 @@ int compute_layout(const sift_shape* s, sift_md_layout* out) {
   out->n_items = (int32_t)(nmb * s->n_q_heads);
   size_t o = 0;
   auto take = [&](int64_t n_int32) { size_t r = o; o = align_up(o + (size_t)n_int32 * 4, 128); return r; };
-  out->tile_base = take(D + 2);
+  out->tile_base = take(dt.n_seg + 1);
   out->tile_seg = take(nt);
   out->tile_row0 = take(nt);
   out->tile_rows = take(nt);
@@ -153,6 +202,9 @@ int compute_layout(const sift_shape* s, sift_md_layout* out) {
   out->sched = take((int64_t)s->n_layers * out->n_items);
   out->counters = take((int64_t)s->n_layers * 2);
   take((int64_t)s->n_layers * out->n_items);   // scheduler keys (private, unnamed: sched_key_offset())
+  out->seg_info = take((int64_t)dt.n_seg * 4);
+  out->n_seg = dt.n_seg;
+  out->n_tokens = dt.off[dt.n_seg];
   out->total_bytes = o;
   return SIFT_OK;
 }
@@ -200,11 +252,7 @@ int sift_decode_metadata(const sift_shape* shape, const uint8_t* la_base, const 
   if (shape->n_docs > 0 && (!la_base || !ca_base || !la_doc_off || !ca_doc_off))
     return set_error(SIFT_ERR_INVALID_ARG, "bit-vector pointer is NULL");
   static thread_local DocTable dt;
-  dt.n_docs = shape->n_docs;
-  dt.query_len = shape->query_len;
-  dt.tile = shape->tile;
-  dt.gran = shape->cross_gran;
-  for (int d = 0; d <= shape->n_docs; ++d) dt.off[d] = shape->doc_offsets[d];
+  build_segments(shape, &dt);
   for (int d = 0; d < shape->n_docs; ++d) {
     if (la_doc_off[d] < 0 || ca_doc_off[d] < 0) return set_error(SIFT_ERR_INVALID_ARG, "negative blob offset at doc %d", d);
     dt.la_off[d] = la_doc_off[d];

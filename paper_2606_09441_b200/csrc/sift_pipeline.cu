@@ -35,7 +35,7 @@ struct HostLayout {
 static int host_layout(const sift_shape* s, size_t la_bytes, size_t ca_bytes, HostLayout* out) {
   int rc = validate_shape(s);
   if (rc) return rc;
-  const int64_t n = (int64_t)s->doc_offsets[s->n_docs] + s->query_len;
+  const int64_t n = shape_n_tokens(s);
   const int hpg = s->n_q_heads / s->n_kv_heads;
   sift_shape sub = *s;
   sub.n_layers = 1; sub.n_q_heads = hpg; sub.n_kv_heads = 1;
@@ -147,7 +147,7 @@ extern "C" int sift_prefill_layer_host(sift_host_ctx* ctx, const sift_shape* sha
   char *qd = ws + hl.q, *kd = ws + hl.k, *vd = ws + hl.v, *od = ws + hl.o;
   float* lsed = reinterpret_cast<float*>(ws + hl.lse);
   uint8_t *lad = reinterpret_cast<uint8_t*>(ws + hl.la), *cad = reinterpret_cast<uint8_t*>(ws + hl.ca);
-  const int64_t n = (int64_t)shape->doc_offsets[D] + shape->query_len;
+  const int64_t n = shape_n_tokens(shape);
   const size_t d2 = (size_t)HD * 2, qp = (size_t)Hq * d2, kp = (size_t)Hkv * d2;   // device row pitches (dense)
   cudaStream_t user = (cudaStream_t)stream;
 
