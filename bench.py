@@ -314,6 +314,8 @@ def run_ours(args):
         extra["density_sweep_32k"] = density_sweep_leg(case, peaks, den_ms, max(3, args.steps // 4))
         extra["paged_32k"] = dict(paged_leg(case, peaks, max(3, args.steps // 4)), row_granular_attention_ms=att_ms,
                                   row_granular_effective_tflops=achieved)
+        extra["batch_8x10k"] = batch_leg(peaks, max(3, args.steps // 4))
+        torch.cuda.empty_cache()
         extra["full_stack"] = full_stack_leg(args.layers, peaks)
 
     out = {
@@ -486,6 +488,93 @@ def paged_leg(base_case, peaks, steps):
             "paged_frac_of_peak": c.flops / (ms * 1e-3) / 1e12 / peaks["bf16"]}
 
 
+def batch_leg(peaks, steps, n_prompts=8):
+    """n_prompts prompts of C2's shape (10 x 1024 + 128) in ONE decode + ONE attention launch, against
+    the same prompts one call each.  One 10K prompt has 32 x 41 work items for 148 persistent CTAs; the batch fills them."""
+    from paper_2606_09441_b200 import api
+    b = wl.config_batch_8x10k() if n_prompts == 8 else wl.make_batch("batch", [wl.config_8b_10k(wl.BASE_SEED + 1000 * (i + 1)) for i in range(n_prompts)])
+    singles = [GpuCase(w, qkv_dev=w.qkv_on_device(0), host=False) for w in b.members]
+    flops = float(sum(c.flops for c in singles))
+    shape = api.Shape.from_batch(b)
+    q, k, v = (torch.cat([getattr(c, n) for c in singles]) for n in ("q", "k", "v"))
+    la, ca = torch.from_numpy(b.la_blob).cuda(), torch.from_numpy(b.ca_blob).cuda()
+    md = torch.empty(api.sift_metadata_size(shape), dtype=torch.uint8, device="cuda")
+    o, lse = torch.empty_like(q), torch.empty((q.shape[1], q.shape[0]), dtype=torch.float32, device="cuda")
+    dec = lambda: api.sift_decode_metadata(shape, la, b.la_doc_off, ca, b.ca_doc_off, md)
+    att = lambda: api.sift_prefill_attention(shape, 0, q, k, v, md, o, lse)
+    def one_by_one():
+        for c in singles:
+            c.attention()
+    dec()
+    for _ in range(3):
+        att(); one_by_one()
+    ms_b = float(np.mean(time_each(att, steps)))
+    ms_s = float(np.mean(time_each(one_by_one, steps)))
+    us_d = float(np.mean(time_each_flushed(dec, steps))) * 1e3
+    return {"prompts": n_prompts, "n_tokens": int(q.shape[0]), "batch_attention_ms": ms_b, "batch_effective_tflops": flops / (ms_b * 1e-3) / 1e12,
+            "batch_frac_of_peak": flops / (ms_b * 1e-3) / 1e12 / peaks["bf16"], "one_call_each_attention_ms": ms_s,
+            "one_call_each_effective_tflops": flops / (ms_s * 1e-3) / 1e12, "batch_decode_us": us_d,
+            "recipe": "%d x (%s), seeds differ" % (n_prompts, b.members[0].recipe)}
+
+
+def run_head_sharded(args):
+    """--shard heads (PAPER.md:L283 TP = 4/8): ONE prompt (the same seed on every rank), rank r
+    takes a contiguous block of kv heads with their q-heads, decodes and attends on its sub-shape and writes its own
+    columns of O.  No collective in the data path; value = flops of all ranks / max-over-ranks step time (strong scaling)."""
+    rank, world, local = dist_setup(args.gpus)
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    from paper_2606_09441_b200 import api, metrics, shard
+    w = wl.CONFIGS[args.config]()
+    ps = w.shape
+    sh = shard.head_shard(ps.n_q_heads, ps.n_kv_heads, rank, world)
+    assert sh.n_kv > 0, "more ranks than kv heads"
+    sub = api.Shape.from_prompt(shard.shard_prompt_shape(ps, sh))
+    la_off, ca_off = shard.shard_blob_offsets(w, sh, 0)
+    la, ca = torch.from_numpy(w.la_blob).cuda(), torch.from_numpy(w.ca_blob).cuda()
+    q, k, v = (t.cuda() for t in w.qkv(0))
+    o = torch.empty_like(q)
+    qs, ks, vs = shard.shard_views(q, k, v, sh)
+    os_ = o[:, sh.q0:sh.q1]
+    lse = torch.empty((sh.n_q, q.shape[0]), dtype=torch.float32, device="cuda")
+    md = torch.empty(api.sift_metadata_size(sub), dtype=torch.uint8, device="cuda")
+
+    def step():
+        api.sift_decode_metadata(sub, la, la_off, ca, ca_off, md)
+        api.sift_prefill_attention(sub, 0, qs, ks, vs, md, os_, lse)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    views = {k_: t.cpu().numpy() for k_, t in api.metadata_views(sub, md).items()}
+    flops = metrics.attention_flops(int(metrics.marked_pairs_per_head(views, 0, ps.n_docs, ps.cross_gran).sum()), ps.head_dim)
+    sampler = ClockSampler(local)
+    launches0 = api.sift_launch_count()
+    barrier(world)
+    torch.cuda.synchronize()
+    sampler.start()
+    ms = time_region(step, args.steps) / args.steps
+    torch.cuda.synchronize()
+    barrier(world)
+    launches = api.sift_launch_count() - launches0
+    clocks = sampler.stop()
+    ms_step = max_over_ranks(ms, world)
+    flops_all = sum_over_ranks(float(flops), world)
+    value = flops_all / (ms_step * 1e-3) / 1e12
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic", "impl": "ours",
+            "config": {"workload": w.name + ": " + w.recipe, "n_tokens": ps.n_tokens, "heads": f"{ps.n_q_heads}/{ps.n_kv_heads}",
+                       "head_dim": ps.head_dim, "l2": "inputs larger than L2, no flush",
+                       "parallelism": f"head-sharded x{world}: rank r owns kv heads [{sh.kv0},{sh.kv1}) style blocks of one prompt, no collective"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "extra": {"rank0_heads": [sh.q0, sh.q1], "rank0_flops": flops}}))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -521,9 +610,13 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra-legs", action="store_true", help="skip the density sweep, paged and full-stack legs")
     ap.add_argument("--layers", type=int, default=32, help="layers of --config full-stack")
+    ap.add_argument("--shard", default="none", choices=["none", "heads"],
+                    help="heads: split ONE prompt's kv-head groups over the ranks (strong scaling, no collective)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.shard == "heads":
+        run_head_sharded(args)
     elif args.config == "full-stack" and args.gpus == 1:
         run_full_stack(args)
     else:
