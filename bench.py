@@ -484,8 +484,24 @@ def paged_leg(base_case, peaks, steps):
     for _ in range(2):
         c.attention()
     ms = float(np.mean(time_each(c.attention, steps)))
-    return {"paged_attention_ms": ms, "paged_effective_tflops": c.flops / (ms * 1e-3) / 1e12, "paged_marked_density": c.flops / c.dense_flops,
-            "paged_frac_of_peak": c.flops / (ms * 1e-3) / 1e12 / peaks["bf16"]}
+    out = {"paged_attention_ms": ms, "paged_effective_tflops": c.flops / (ms * 1e-3) / 1e12, "paged_marked_density": c.flops / c.dense_flops,
+           "paged_frac_of_peak": c.flops / (ms * 1e-3) / 1e12 / peaks["bf16"]}
+    # the paper's replicated per-(head, M-block) list rebuilt from MD-v1, beside MD-v1 itself
+    for name, case in (("paper_indices_G=T", c), ("paper_indices_G=1", base_case)):
+        api = case.api
+        ptr = api.sift_paper_index_offsets(case.shape, 0, case.md)
+        tot = ptr[:, -1].cpu()
+        idx = torch.empty((case.shape.n_q_heads, int(tot.max())), dtype=torch.int32, device="cuda")
+        def export():
+            api.sift_paper_index_offsets(case.shape, 0, case.md)
+            api.sift_export_paper_indices(case.shape, 0, case.md, ptr, idx)
+        export()
+        us = float(np.mean(time_each(export, steps))) * 1e3
+        dus = float(np.mean(time_each_flushed(case.decode, steps))) * 1e3
+        out[name] = {"paper_layout_bytes": int(tot.sum()) * 4 + ptr.numel() * 8, "md_v1_bytes": int(case.decode_bytes),
+                     "export_us": us, "md_v1_decode_us": dus}
+        del idx
+    return out
 
 
 def batch_leg(peaks, steps, n_prompts=8):

@@ -183,6 +183,21 @@ int sift_encode_document(int32_t doc_len, int32_t n_q_heads, int32_t n_kv_heads,
                          const float* lse, float alpha, float beta, float gamma, float softmax_scale,
                          uint8_t* la_out, uint8_t* ca_out, void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- the paper's own index layout (sec 5.1) ----
+ * sparse_n_indices as the paper stores it: per (head, M-block t) ONE packed int32 list, the CA entries of all earlier
+ * documents of the prompt first (key rows at G = 1, global tile ids at G = tile), then the M-block's LA entries (global
+ * tile ids); a query M-block lists its causal N-blocks.  MD-v1 keeps the CA entries of a head once; these two calls
+ * rebuild the replicated layout from a decoded metadata buffer, for one layer, on `stream`:
+ *   sift_paper_index_offsets   ptr (dev, out) [n_q_heads][NT + 1] int64: ptr[h][t] = entries of the M-blocks before t,
+ *                              ptr[h][NT] = entries of head h (read it back to size idx).
+ *   sift_export_paper_indices  idx (dev, out) [n_q_heads][head_stride] int32: the list of (h, t) at
+ *                              idx[h * head_stride + ptr[h][t] ..]; entries at or beyond head_stride are not written.
+ * NT = sift_md_layout.n_tiles (an M-block here is one query tile of `tile` rows). */
+int sift_paper_index_offsets(const sift_shape* shape, int32_t layer, const void* metadata /*dev*/, int64_t* ptr /*dev*/,
+                             void* stream);
+int sift_export_paper_indices(const sift_shape* shape, int32_t layer, const void* metadata /*dev*/,
+                              const int64_t* ptr /*dev*/, int32_t* idx /*dev*/, int64_t head_stride, void* stream);
+
 /* Number of kernels the library has launched in this process (bench.py's gpu_launches). */
 int64_t sift_launch_count(void);
 

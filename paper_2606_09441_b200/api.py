@@ -17,7 +17,7 @@ EXPORTS = ("sift_version", "sift_last_error", "sift_metadata_size", "sift_metada
            "sift_decode_metadata", "sift_prefill_attention", "sift_dense_causal_attention", "sift_launch_count",
            "sift_encode_workspace_size", "sift_encode_output_sizes", "sift_encode_document",
            "sift_host_ctx_create", "sift_host_ctx_destroy", "sift_prefill_layer_host_workspace_size",
-           "sift_prefill_layer_host")
+           "sift_prefill_layer_host", "sift_paper_index_offsets", "sift_export_paper_indices")
 
 
 class SiftShape(C.Structure):
@@ -78,6 +78,9 @@ def lib() -> C.CDLL:
                                               C.c_void_p, C.c_size_t, C.POINTER(C.c_int64),
                                               C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64,
                                               C.c_void_p, C.c_int64, C.c_void_p, C.c_float, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.sift_paper_index_offsets.argtypes = [C.POINTER(SiftShape), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.sift_export_paper_indices.argtypes = [C.POINTER(SiftShape), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                                C.c_int64, C.c_void_p]
         _lib = L
     return _lib
 
@@ -313,3 +316,21 @@ def sift_prefill_layer_host(ctx: HostContext, shape: Shape, layer: int, la_h: to
                                        lse_h.data_ptr() if lse_h is not None else None, float(softmax_scale),
                                        workspace.data_ptr(), workspace.numel(), _stream(stream))
     _check(rc, "sift_prefill_layer_host")
+
+
+def sift_paper_index_offsets(shape: Shape, layer: int, metadata: torch.Tensor, stream=None) -> torch.Tensor:
+    """int64 CUDA tensor [n_q_heads, NT + 1] (include/sift.h: the paper's per-(head, M-block) list offsets)."""
+    nt = sift_metadata_layout(shape).n_tiles
+    ptr = torch.empty((shape.n_q_heads, nt + 1), dtype=torch.int64, device=metadata.device)
+    _check(lib().sift_paper_index_offsets(C.byref(shape.c), layer, metadata.data_ptr(), ptr.data_ptr(), _stream(stream)),
+           "sift_paper_index_offsets")
+    return ptr
+
+
+def sift_export_paper_indices(shape: Shape, layer: int, metadata: torch.Tensor, ptr: torch.Tensor, idx: torch.Tensor,
+                              stream=None) -> torch.Tensor:
+    """idx: int32 CUDA tensor [n_q_heads, head_stride], sized by the caller from ptr[:, -1]."""
+    assert idx.is_cuda and idx.dtype == torch.int32 and idx.dim() == 2 and idx.stride(1) == 1
+    _check(lib().sift_export_paper_indices(C.byref(shape.c), layer, metadata.data_ptr(), ptr.data_ptr(), idx.data_ptr(),
+                                           idx.stride(0), _stream(stream)), "sift_export_paper_indices")
+    return idx

@@ -9,7 +9,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libsift_b200.so")
-SOURCES = ["sift_host.cu", "sift_decode.cu", "sift_attention.cu", "sift_encode.cu", "sift_pipeline.cu"]
+SOURCES = ["sift_host.cu", "sift_decode.cu", "sift_attention.cu", "sift_encode.cu", "sift_pipeline.cu", "sift_export.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-shared", "-Xcompiler", "-fPIC",

@@ -452,3 +452,29 @@ def test_set_device_round_trip():
     torch.cuda.set_device(0)
     _, _, o2, l2 = gu.run_sift(w)
     assert torch.equal(o1, o2) and torch.equal(l1, l2)
+
+
+@pytest.mark.parametrize("gran,tile", [(1, 64), (64, 64), (128, 128)])
+def test_paper_index_export_matches_oracle_paper_view(gran, tile):
+    """SURVEY 8(f)-2 / PAPER.md:L239-245: the per-(head, M-block) list the paper's kernel consumes, rebuilt on the GPU
+    from MD-v1, equals oracle.paper_view entry for entry; its offsets are the running list lengths."""
+    w = wl.custom("pv", n_layers=2, n_q_heads=4, n_kv_heads=2, head_dim=64, doc_lens=(300, 64, 1, 517), query_len=150, tile=tile,
+                  cross_gran=gran, p_loc=0.4, p_cross=0.3, seed=41)
+    shape, md = gu.decode_on_gpu(w)
+    ref = gu.oracle_md(w)
+    nt = int(ref["NT"])
+    for layer in range(2):
+        ptr = api.sift_paper_index_offsets(shape, layer, md)
+        total = int(ptr[:, -1].max())
+        idx = torch.full((shape.n_q_heads, total + 7), -7, dtype=torch.int32, device="cuda")
+        api.sift_export_paper_indices(shape, layer, md, ptr, idx)
+        torch.cuda.synchronize()
+        ptr_h, idx_h = ptr.cpu().numpy(), idx.cpu().numpy()
+        for h in range(shape.n_q_heads):
+            pos = 0
+            for t in range(nt):
+                lst = so.paper_view(ref, layer, h, t)
+                assert ptr_h[h, t] == pos
+                assert np.array_equal(idx_h[h, pos: pos + len(lst)], lst), (layer, h, t)
+                pos += len(lst)
+            assert ptr_h[h, nt] == pos and np.all(idx_h[h, pos:] == -7)     # nothing written past the head's entries
