@@ -44,7 +44,8 @@ struct DecodeParams {
   int32_t cross_parts;    // CTAs per (layer, head) for the cross list: 4 when the grid would not fill the GPU, else 1
   int32_t tile_shift, gran_shift;   // tile and cross_gran are powers of two (64 | 128; 1 | tile): no integer divisions
   int32_t done_base;      // first slot of this call in g_layer_done
-  int32_t split_keys;     // 1: a separate CTA per (layer, head) computes the scheduler keys
+  int32_t fused;          // 1 (small grids): the scheduler runs inside this launch (a key CTA per (layer, head), the
+                          // layer's last CTA sorts); 0 (whole stacks): sift_schedule_kernel follows
 };
 
 // exclusive scan over the block; returns the exclusive prefix of v and (via total) the block sum
@@ -243,10 +244,9 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
   // (and, for the first head, the tile tables).  Shortens the latency chain of a CTA (a single layer is latency-bound).
   const int kCrossParts = p.cross_parts;
   const bool do_cross = ((int)blockIdx.z < kCrossParts);
-  // the scheduler keys of the head come from the local-list CTA, or, when the grid is small (split_keys), from a CTA
-  // of their own (z = kCrossParts + 1) so that the call's critical path is shorter
+  // fused scheduler (small grids): the sort keys of the head's work items come from a CTA of their own (z = kCrossParts + 1)
   const bool do_local = ((int)blockIdx.z == kCrossParts);
-  const bool do_keys = p.split_keys ? ((int)blockIdx.z == kCrossParts + 1) : do_local;
+  const bool do_keys = p.fused && ((int)blockIdx.z == kCrossParts + 1);
   const bool writer = (h == 0 && l == 0 && do_local);
   if (writer) {
     for (int d = tid; d <= S; d += kDecodeThreads) p.tile_base[d] = s_tile_base[d];
@@ -527,6 +527,7 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
   // ---- scheduler (a5), fused: the CTA that finishes a layer last sorts the layer's work items (head, M-block) by
   // key = (kv-head group, descending cost) with a counting sort in shared memory; the persistent attention grid pulls
   // them through an atomic counter.  The keys of the other CTAs are published by the fence + counter below.
+  if (!p.fused) return;
   __shared__ int s_last;
   __threadfence();
   __syncthreads();
@@ -577,6 +578,72 @@ sift_decode_kernel(const __grid_constant__ DocTable dt, const DecodeParams p) {
   }
 }
 
+// Scheduler as a launch of its own (whole stacks, p.fused == 0): one 1024-thread CTA per layer computes the same sort
+// keys from the decoded counts and counting-sorts the layer's work items.
+constexpr int kSchedThreads = 1024;
+__global__ void __launch_bounds__(kSchedThreads)
+sift_schedule_kernel(const DecodeParams p, int n_docs) {
+  __shared__ int s_hist[kCostBuckets];
+  __shared__ int s_scan[kSchedThreads / 32 + 1];
+  constexpr int NQ = SIFT_Q_TILES_PER_ITEM;
+  const int l = blockIdx.x, tid = threadIdx.x;
+  const int D = n_docs, NT = p.n_tiles, NMB = p.n_mblocks;
+  for (int i = tid; i < kCostBuckets; i += kSchedThreads) s_hist[i] = 0;
+  __syncthreads();
+  const int groups = (p.n_kv_heads + p.kv_per_group - 1) / p.kv_per_group, bpg = kCostBuckets / groups;
+  auto key_of = [&](int e) {
+    const int h = e / NMB, mb = e - h * NMB;
+    const int64_t lh = (int64_t)l * p.n_q_heads + h;
+    const int t0 = p.mblock_tile0[mb], t1 = min(p.mblock_tile0[mb + 1], t0 + NQ);
+    const int4 si = reinterpret_cast<const int4*>(p.seg_info)[p.tile_seg[t0]];
+    int c = 0;
+    if (si.x >= 0) {
+      const int cp = p.cross_ptr[lh * (D + 1) + si.x] - p.cross_ptr[lh * (D + 1) + si.y];
+      const int cross_steps = (p.gran == 1) ? (cp + 127) >> 7 : cp;
+      for (int t = t0; t < t1; ++t) c += cross_steps + p.local_cnt[lh * NT + t];
+    } else {
+      for (int t = t0; t < t1; ++t) c += (p.tile_row0[t] - si.z + p.tile_rows[t] + 127) >> 7;
+    }
+    const int g = h / (p.n_q_heads / p.n_kv_heads) / p.kv_per_group;
+    return g * bpg + (bpg - 1 - min(c, bpg - 1));
+  };
+  // the key of an item is a chain of dependent global loads: evaluate it once and keep it in registers for the
+  // scatter pass (up to kCached items per thread; larger layers recompute)
+  constexpr int kCached = 8;
+  int ck[kCached];
+#pragma unroll
+  for (int k = 0; k < kCached; ++k) {
+    const int e = tid + k * kSchedThreads;
+    ck[k] = (e < p.n_items) ? key_of(e) : 0;
+  }
+#pragma unroll
+  for (int k = 0; k < kCached; ++k)
+    if (tid + k * kSchedThreads < p.n_items) atomicAdd(&s_hist[ck[k]], 1);
+  for (int e = tid + kCached * kSchedThreads; e < p.n_items; e += kSchedThreads) atomicAdd(&s_hist[key_of(e)], 1);
+  __syncthreads();
+  {  // exclusive scan over buckets (bucket 0 = first to be processed)
+    constexpr int PER = kCostBuckets / kSchedThreads;
+    int loc[PER], sum = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { loc[k] = s_hist[tid * PER + k]; sum += loc[k]; }
+    int tot;
+    int ex = block_exclusive_scan<kSchedThreads>(sum, s_scan, tot);
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { s_hist[tid * PER + k] = ex; ex += loc[k]; }
+  }
+  __syncthreads();
+  int32_t* sched = p.sched + (int64_t)l * p.n_items;
+  auto place = [&](int e, int b) {
+    const int h = e / NMB;
+    sched[atomicAdd(&s_hist[b], 1)] = (h << 20) | (e - h * NMB);
+  };
+#pragma unroll
+  for (int k = 0; k < kCached; ++k)
+    if (tid + k * kSchedThreads < p.n_items) place(tid + k * kSchedThreads, ck[k]);
+  for (int e = tid + kCached * kSchedThreads; e < p.n_items; e += kSchedThreads) place(e, key_of(e));
+  if (tid < 2) p.counters[l * 2 + tid] = 0;
+}
+
 int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable& dt, const uint8_t* la_base,
                   const uint8_t* ca_base, void* md, cudaStream_t st) {
   if (lay.n_mblocks >= (1 << 20)) return set_error(SIFT_ERR_UNSUPPORTED, "too many M-blocks");
@@ -599,17 +666,21 @@ int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable
   int num_sms = 0;
   if (int rc = device_sm_count(&num_sms)) return rc;
   p.cross_parts = ((int64_t)s->n_q_heads * s->n_layers <= num_sms) ? kMaxCrossParts : 1;
-  p.split_keys = (p.cross_parts > 1);
+  // one layer: a second launch would double the latency of the call, so the scheduler is fused (21 vs 26 us at 32K);
+  // whole stacks: the recount behind the keys and the per-layer sort tails cost more than a second launch that sorts
+  // all layers in parallel (32 layers of C3: 66 us fused, 50 us with the separate kernel)
+  p.fused = (p.cross_parts > 1);
   p.kv_per_group = sched_kv_heads_per_group(lay.n_tokens, s->head_dim, s->n_kv_heads);
   p.tile_shift = (s->tile == 128) ? 7 : 6;
   p.gran_shift = (s->cross_gran == 1) ? 0 : p.tile_shift;
   if (s->n_layers > kDoneRing / 4) return set_error(SIFT_ERR_UNSUPPORTED, "too many layers in one decode call");
   p.done_base = (int32_t)(g_done_ticket.fetch_add((uint32_t)s->n_layers, std::memory_order_relaxed) % kDoneRing);
   cudaGetLastError();
-  sift_decode_kernel<<<dim3(s->n_q_heads, s->n_layers, p.cross_parts + 1 + p.split_keys), kDecodeThreads, 0, st>>>(dt, p);
+  sift_decode_kernel<<<dim3(s->n_q_heads, s->n_layers, p.cross_parts + 1 + p.fused), kDecodeThreads, 0, st>>>(dt, p);
+  if (!p.fused) sift_schedule_kernel<<<s->n_layers, kSchedThreads, 0, st>>>(p, s->n_docs);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "decode launch: %s", cudaGetErrorString(e));
-  count_launch(1);
+  count_launch(p.fused ? 1 : 2);
   return SIFT_OK;
 }
 

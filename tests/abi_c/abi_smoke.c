@@ -109,7 +109,7 @@ static int gpu_part(void) {
       }
     }
   }
-  CHECK(sift_launch_count() >= 3);
+  CHECK(sift_launch_count() >= 3); /* decode (1 launch when the scheduler is fused) + attention + dense */
   /* the same layer from HOST buffers through sift_prefill_layer_host: host -> host, bit-identical to the single call */
   {
     void *p_la, *p_ca, *p_q, *p_k, *p_v, *p_o, *p_lse, *d_ws, *st;
