@@ -19,6 +19,8 @@ What it is: the plain definitions, written out.
   Part 4  ``encode_document``    -- offline metadata generation (L201, L209, L223).
   Part 5  ``*_batch``            -- several prompts in one call: a loop over prompts around Parts 1-3, shifted to
                                     batch coordinates (container "MD-v1b").
+  Part 6  ``*_fp8``              -- e4m3 Q/K/V with per-head scales: decode the bytes by the format's definition, then
+                                    Part 2 (reading R7).
 
 Readings of the paper where it is silent or garbled are listed in DESIGN.md section 3
 (A1..A26 of SURVEY.md 8(c)); the ones used here are cited inline.
@@ -587,6 +589,40 @@ def sift_attention_rows_batch(q: torch.Tensor, k: torch.Tensor, v: torch.Tensor,
         o_out[sel] = o
         l_out[sel] = lse
     return o_out, l_out
+
+
+# ------------------------------------------------------------------------------------------
+# Part 6: FP8 (e4m3) Q/K/V (sec 2.6 points at FP8/FP4 prefill)
+# ------------------------------------------------------------------------------------------
+# The paper fixes nothing here.  Definition (reading R7): Q, K, V arrive as OCP e4m3 bytes (1 sign, 4 exponent
+# bits with bias 7, 3 mantissa bits; no infinities, S.1111.111 = NaN, largest finite 448) with one fp32 scale per q-head
+# for Q and per kv-head for K and V.  The attention is Part 2's on the DEQUANTISED values q_scale[h] * Q8, k_scale[g] * K8,
+# v_scale[g] * V8: the oracle decodes the bytes by the format's definition and calls Part 2 unchanged (fp64 on
+# request).  What the GPU adds on top (P rounded to e4m3 before P*V) is an approximation the oracle does not imitate;
+# its bound is derived in DESIGN.md and written into the parity test.
+
+def e4m3_decode(b: np.ndarray) -> np.ndarray:
+    """uint8 -> float64 by the OCP FP8 E4M3 definition: (-1)^s * 2^(e-7) * (1 + m/8) for e > 0, (-1)^s * 2^-6 * m/8
+    for e = 0; e = 15, m = 7 is NaN."""
+    b = np.asarray(b, np.uint8).astype(np.int64)
+    sgn = np.where(b & 0x80, -1.0, 1.0)
+    e, m = (b >> 3) & 0xF, b & 0x7
+    val = np.where(e > 0, np.ldexp(1.0 + m / 8.0, e - 7), np.ldexp(m / 8.0, -6))
+    val = np.where((e == 15) & (m == 7), np.nan, val)
+    return sgn * val
+
+
+def sift_attention_rows_fp8(q8: np.ndarray, k8: np.ndarray, v8: np.ndarray, q_scale: Sequence[float], k_scale: Sequence[float],
+                            v_scale: Sequence[float], head: int, doc_offsets: Sequence[int], query_len: int, tile: int,
+                            gran: int, la_vecs: Sequence[np.ndarray], ca_vecs: Sequence[np.ndarray], rows: Sequence[int],
+                            scale: Optional[float] = None, dtype: torch.dtype = torch.float32) -> Tuple[torch.Tensor, torch.Tensor]:
+    """q8 [N,Hq,d], k8, v8 [N,Hkv,d] uint8 (e4m3 bytes).  Dequantise, then Part 2 as it stands."""
+    hq, hkv = q8.shape[1], k8.shape[1]
+    q = torch.from_numpy(e4m3_decode(q8) * np.asarray(q_scale, np.float64)[None, :, None]).to(dtype)
+    k = torch.from_numpy(e4m3_decode(k8) * np.asarray(k_scale, np.float64)[None, :, None]).to(dtype)
+    v = torch.from_numpy(e4m3_decode(v8) * np.asarray(v_scale, np.float64)[None, :, None]).to(dtype)
+    assert q.shape[1] == hq and k.shape[1] == hkv
+    return sift_attention_rows(q, k, v, head, doc_offsets, query_len, tile, gran, la_vecs, ca_vecs, rows, scale=scale, dtype=dtype)
 
 
 # ------------------------------------------------------------------------------------------

@@ -330,6 +330,17 @@ def stack_orderings(w: Workload, n: int = 4) -> List[List[int]]:
     return out
 
 
+def quantize_e4m3(x: torch.Tensor, per_head_amax: float = 448.0) -> Tuple[torch.Tensor, np.ndarray]:
+    """Input plumbing for the FP8 variant: x [N, H, d] float -> (uint8 e4m3 bytes [N, H, d], fp32
+    scale per head) with scale[h] = max|x[:, h]| / per_head_amax, so that x ~ scale[h] * decode(bytes).  Rounding is the
+    library conversion of torch (round to nearest even); values are clamped to the format's range first."""
+    xf = x.float()
+    amax = xf.abs().amax(dim=(0, 2)).clamp_min(1e-12)
+    scale = (amax / per_head_amax)
+    y = (xf / scale[None, :, None]).clamp(-448.0, 448.0).to(torch.float8_e4m3fn)
+    return y.view(torch.uint8), scale.numpy().astype(np.float32)
+
+
 @dataclass
 class BatchWorkload:
     """Several prompts packed back to back on the token axis: prompt p = its documents, then its

@@ -505,3 +505,47 @@ def test_batch_attention_rows_against_brute_force():
             ob, lb = so.brute_force_row(q[r, h].double().numpy(), k[:, kvh].double().numpy(), v[:, kvh].double().numpy(),
                                         allowed, 1.0 / math.sqrt(sh.head_dim))
             assert np.allclose(o[ri].numpy(), ob, atol=1e-9) and abs(float(lse[ri]) - lb) < 1e-9
+
+
+# ---------------------------------------------------------------- FP8 (e4m3) inputs
+
+def test_e4m3_decode_format_values():
+    """OCP FP8 E4M3 by hand: 0x38 = 1.0, 0x7E = 448 (largest finite), 0x01 = 2^-9 (smallest subnormal), 0x08 = 2^-6
+    (smallest normal), 0x3C = 1.5, 0xC0 = -2, 0x00 / 0x80 = +-0, 0x7F = NaN; and the whole table against torch."""
+    got = so.e4m3_decode(np.array([0x38, 0x7E, 0x01, 0x08, 0x3C, 0xC0, 0x00, 0x80], np.uint8))
+    assert list(got) == [1.0, 448.0, 2.0 ** -9, 2.0 ** -6, 1.5, -2.0, 0.0, -0.0]
+    assert np.isnan(so.e4m3_decode(np.array([0x7F, 0xFF], np.uint8))).all()
+    allb = np.arange(256, dtype=np.uint8)
+    ref = torch.from_numpy(allb).view(torch.float8_e4m3fn).to(torch.float64).numpy()
+    ok = ~np.isnan(ref)
+    assert np.array_equal(so.e4m3_decode(allb)[ok], ref[ok]) and np.isnan(so.e4m3_decode(allb)[~ok]).all()
+    # strictly increasing over the positive finite codes: 127 distinct magnitudes
+    assert np.all(np.diff(so.e4m3_decode(np.arange(0, 0x7F, dtype=np.uint8))) > 0)
+
+
+def test_fp8_attention_is_attention_of_the_dequantised_values_and_scales_fold():
+    w = wl.custom("f8", n_layers=1, n_q_heads=2, n_kv_heads=1, head_dim=64, doc_lens=(100, 70), query_len=30, tile=64, seed=9)
+    sh = w.shape
+    q, k, v = w.qkv(0)
+    q8, qs = wl.quantize_e4m3(q)
+    k8, ks = wl.quantize_e4m3(k)
+    v8, vs = wl.quantize_e4m3(v)
+    rows = [0, 63, 64, 99, 100, 169, 170, 199]
+    for h in range(2):
+        la, ca = so.head_vectors(w, 0, h)
+        o, lse = so.sift_attention_rows_fp8(q8.numpy(), k8.numpy(), v8.numpy(), qs, ks, vs, h, sh.doc_offsets, sh.query_len,
+                                            sh.tile, 1, la, ca, rows, dtype=torch.float64)
+        # (a) the same rows from explicitly dequantised tensors through Part 2
+        qd = q8.view(torch.float8_e4m3fn).double() * torch.from_numpy(qs.astype(np.float64))[None, :, None]
+        kd = k8.view(torch.float8_e4m3fn).double() * torch.from_numpy(ks.astype(np.float64))[None, :, None]
+        vd = v8.view(torch.float8_e4m3fn).double() * torch.from_numpy(vs.astype(np.float64))[None, :, None]
+        o2, lse2 = so.sift_attention_rows(qd, kd, vd, h, sh.doc_offsets, sh.query_len, sh.tile, 1, la, ca, rows, dtype=torch.float64)
+        assert torch.allclose(o, o2, atol=1e-12) and torch.allclose(lse, lse2, atol=1e-12)
+        # (b) a factor moved from q_scale to the softmax scale changes nothing; v_scale is linear in O
+        o3, lse3 = so.sift_attention_rows_fp8(q8.numpy(), k8.numpy(), v8.numpy(), qs * 2, ks, vs * 3, h, sh.doc_offsets, sh.query_len,
+                                              sh.tile, 1, la, ca, rows, scale=0.5 / math.sqrt(64), dtype=torch.float64)
+        assert torch.allclose(o3, 3 * o, atol=1e-9) and torch.allclose(lse3, lse, atol=1e-9)
+        # (c) quantisation is the only difference from the bf16 path: close to the unquantised result (e4m3: 2^-4 relative)
+        o4, _ = so.sift_attention_rows(q.double(), k.double(), v.double(), h, sh.doc_offsets, sh.query_len, sh.tile, 1, la, ca, rows,
+                                       dtype=torch.float64)
+        assert float((o - o4).abs().max()) < 0.5
