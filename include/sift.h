@@ -123,6 +123,19 @@ int sift_prefill_attention(const sift_shape* shape, int32_t layer,
                            const void* metadata /*dev, from sift_decode_metadata*/,
                            void* O, int64_t o_row_stride, float* lse, float softmax_scale, void* stream);
 
+/* FP8 variant (sec 2.6 points at FP8 prefill; reading R7).  Q8 [N][n_q_heads][128], K8, V8
+ * [N][n_kv_heads][128]: OCP e4m3 bytes, dev, row strides in elements (= bytes), bases and strides 16-byte aligned;
+ * q_scale HOST [n_q_heads], k_scale / v_scale HOST [n_kv_heads], all > 0.  The result is sift_prefill_attention of the
+ * dequantised values q_scale[h] * Q8, k_scale[g] * K8, v_scale[g] * V8 (O bf16, lse fp32 as there), computed with
+ * kind::f8f6f4 tensor-core MMAs: the logits are exact products accumulated in fp32, P is rounded to e4m3 before P*V
+ * (tolerance in DESIGN.md).  head_dim 128 only (SIFT_ERR_UNSUPPORTED otherwise).  Same metadata, same ordering rule. */
+int sift_prefill_attention_fp8(const sift_shape* shape, int32_t layer,
+                               const void* Q8, const void* K8, const void* V8,
+                               int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
+                               const float* q_scale /*HOST*/, const float* k_scale /*HOST*/, const float* v_scale /*HOST*/,
+                               const void* metadata /*dev*/, void* O, int64_t o_row_stride, float* lse,
+                               float softmax_scale, void* stream);
+
 /* Dense causal attention over n_tokens rows with the same kernel body (no metadata).  Calls may be in flight on
  * different streams at the same time: each call draws its own work counter (cleared on `stream` before the launch). */
 int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,

@@ -17,7 +17,8 @@ EXPORTS = ("sift_version", "sift_last_error", "sift_metadata_size", "sift_metada
            "sift_decode_metadata", "sift_prefill_attention", "sift_dense_causal_attention", "sift_launch_count",
            "sift_encode_workspace_size", "sift_encode_output_sizes", "sift_encode_document",
            "sift_host_ctx_create", "sift_host_ctx_destroy", "sift_prefill_layer_host_workspace_size",
-           "sift_prefill_layer_host", "sift_paper_index_offsets", "sift_export_paper_indices")
+           "sift_prefill_layer_host", "sift_paper_index_offsets", "sift_export_paper_indices",
+           "sift_prefill_attention_fp8")
 
 
 class SiftShape(C.Structure):
@@ -81,6 +82,10 @@ def lib() -> C.CDLL:
         L.sift_paper_index_offsets.argtypes = [C.POINTER(SiftShape), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
         L.sift_export_paper_indices.argtypes = [C.POINTER(SiftShape), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                                 C.c_int64, C.c_void_p]
+        L.sift_prefill_attention_fp8.argtypes = [C.POINTER(SiftShape), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                                 C.c_int64, C.c_int64, C.c_int64, C.POINTER(C.c_float), C.POINTER(C.c_float),
+                                                 C.POINTER(C.c_float), C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p,
+                                                 C.c_float, C.c_void_p]
         _lib = L
     return _lib
 
@@ -334,3 +339,24 @@ def sift_export_paper_indices(shape: Shape, layer: int, metadata: torch.Tensor, 
     _check(lib().sift_export_paper_indices(C.byref(shape.c), layer, metadata.data_ptr(), ptr.data_ptr(), idx.data_ptr(),
                                            idx.stride(0), _stream(stream)), "sift_export_paper_indices")
     return idx
+
+
+def sift_prefill_attention_fp8(shape: Shape, layer: int, q8: torch.Tensor, k8: torch.Tensor, v8: torch.Tensor,
+                               q_scale, k_scale, v_scale, metadata: torch.Tensor, out: Optional[torch.Tensor] = None,
+                               lse: Optional[torch.Tensor] = None, softmax_scale: float = 0.0, stream=None
+                               ) -> Tuple[torch.Tensor, torch.Tensor]:
+    """q8 [N, Hq, 128], k8, v8 [N, Hkv, 128]: uint8 CUDA tensors holding e4m3 bytes; scales: float32 host arrays."""
+    for t in (q8, k8, v8):
+        assert t.is_cuda and t.dtype == torch.uint8 and t.dim() == 3 and t.stride(2) == 1 and t.stride(1) == t.shape[2]
+    if out is None:
+        out = torch.empty(q8.shape, dtype=torch.bfloat16, device=q8.device)
+    if lse is None:
+        lse = torch.empty((q8.shape[1], q8.shape[0]), dtype=torch.float32, device=q8.device)
+    fp = C.POINTER(C.c_float)
+    qs, ks, vs = (np.ascontiguousarray(a, dtype=np.float32) for a in (q_scale, k_scale, v_scale))
+    rc = lib().sift_prefill_attention_fp8(C.byref(shape.c), layer, q8.data_ptr(), k8.data_ptr(), v8.data_ptr(),
+                                          q8.stride(0), k8.stride(0), v8.stride(0), qs.ctypes.data_as(fp),
+                                          ks.ctypes.data_as(fp), vs.ctypes.data_as(fp), metadata.data_ptr(),
+                                          out.data_ptr(), out.stride(0), lse.data_ptr(), float(softmax_scale), _stream(stream))
+    _check(rc, "sift_prefill_attention_fp8")
+    return out, lse

@@ -78,14 +78,17 @@ struct AttnParams {
   float scale_log2;
 };
 
-template <int HD>
+// EB = bytes per Q/K/V element: 2 = bf16 (kind::f16), 1 = e4m3 (kind::f8f6f4, reading R7)
+template <int HD, int EB = 2>
 struct Smem {
-  static constexpr int kHalves = HD / 64;
-  static constexpr int kTileBytes = kBN * HD * 2;          // one K or V tile / one Q tile
+  static_assert(HD * EB % 128 == 0, "a tile row is a whole number of 128-byte swizzle rows");
+  static constexpr int kHalves = HD * EB / 128;            // 128-byte column blocks of a tile
+  static constexpr int kHalfElems = 128 / EB;              // elements per block row
+  static constexpr int kTileBytes = kBN * HD * EB;         // one K or V tile / one Q tile
   // d = 128: 5 stages of 32 KB fit beside the two Q tiles; 2 K + 3 V measured 1-3% faster than 3 K + 2 V (a V stage is
   // held from the P V of one step to the end of the next, a K stage only across its own Q K^T)
-  static constexpr int kKStages = (HD == 128 ? 2 : 4);
-  static constexpr int kVStages = (HD == 128 ? 3 : 4);
+  static constexpr int kKStages = (kTileBytes == 32768 ? 2 : 4);
+  static constexpr int kVStages = (kTileBytes == 32768 ? 3 : 4);
   static constexpr int kQOff = 0;
   static constexpr int kKOff = kQOff + kNQ * kTileBytes;
   static constexpr int kVOff = kKOff + kKStages * kTileBytes;
@@ -164,39 +167,49 @@ __device__ __forceinline__ int dense_steps(int row0, int rows) { return rows > 0
 // ------------------------------------------------------------------------------------------------
 // descriptors
 // ------------------------------------------------------------------------------------------------
-// Q / K tile in smem: HD/64 halves of [128 rows x 128 B], 128-byte swizzle (what TMA writes).  K-chunk k (16 bf16):
-template <int HD>
+// Q / K tile in smem: blocks of [128 rows x 128 B], 128-byte swizzle (what TMA writes).  K-chunk k = 32 bytes of a row
+// (16 bf16 or 32 e4m3 = one MMA's K):
 __device__ __forceinline__ uint64_t kmajor_desc(uint32_t tile_addr, int k) {
   return umma_desc_sw128(tile_addr + (k >> 2) * (kBN * 128) + (k & 3) * 32, 16, 1024);
 }
-// V tile, same smem image, used MN-major (N = head dim contiguous): K-chunk k = 16 key rows = 2 KB further
-template <int HD>
+// V tile, same smem image, used MN-major (N = head dim contiguous): K-chunk k = the key rows of one MMA (16 bf16 rows =
+// 2 KB, 32 e4m3 rows = 4 KB), column blocks kBN * 128 bytes apart
+template <int EB>
 __device__ __forceinline__ uint64_t v_desc(uint32_t tile_addr, int k) {
-  return umma_desc_sw128(tile_addr + k * 2048, kBN * 128, 1024);
+  return umma_desc_sw128(tile_addr + k * (4096 / EB), kBN * 128, 1024);
 }
 
 // compile-time unrolled issue loops (the TMEM offsets must be immediates)
-template <int HD, int Q, int ACC, int K, int KEND>
+// (K counts MMA K-steps: 16 keys (bf16) or 32 keys (e4m3) of P = 8 TMEM columns either way)
+template <int EB, int Q, int ACC, int K, int KEND>
 __device__ __forceinline__ void issue_pv(uint32_t tz, uint32_t vt, uint32_t idesc) {
   if constexpr (K < KEND) {
-    umma_ts_off<256 + Q * 128, Q * 128 + K * 8>(tz, v_desc<HD>(vt, K), idesc, (ACC) | (K > 0));
-    issue_pv<HD, Q, ACC, K + 1, KEND>(tz, vt, idesc);
+    umma_ts_off<256 + Q * 128, Q * 128 + K * 8, EB == 1>(tz, v_desc<EB>(vt, K), idesc, (ACC) | (K > 0));
+    issue_pv<EB, Q, ACC, K + 1, KEND>(tz, vt, idesc);
   }
 }
-template <int HD, int Q, int K = 0>
+template <int HD, int EB, int Q, int K = 0>
 __device__ __forceinline__ void issue_qk(uint32_t tz, uint32_t qt, uint32_t kt, uint32_t idesc) {
-  if constexpr (K < HD / 16) {
-    umma_ss_off<Q * 128>(tz, kmajor_desc<HD>(qt, K), kmajor_desc<HD>(kt, K), idesc, K > 0);
-    issue_qk<HD, Q, K + 1>(tz, qt, kt, idesc);
+  if constexpr (K < HD * EB / 32) {
+    umma_ss_off<Q * 128, EB == 1>(tz, kmajor_desc(qt, K), kmajor_desc(kt, K), idesc, K > 0);
+    issue_qk<HD, EB, Q, K + 1>(tz, qt, kt, idesc);
   }
 }
 
-template <int HD>
-__global__ void __launch_bounds__(kNumThreads, 1)
-sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
-                      const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_kg,
-                      const __grid_constant__ CUtensorMap tm_vg, const AttnParams p) {
-  using S = Smem<HD>;
+// e4m3 path: per-q-head factors (kernel parameter, by value): logits scale in log2 units and the scale of V
+struct F8Scales {
+  float qk_log2[256];   // softmax_scale * log2(e) * q_scale[h] * k_scale[kv(h)]
+  float v[256];         // v_scale[kv(h)]
+};
+constexpr float kP8Shift = 64.f;             // e4m3 P is stored as 2^6 P: weights down to 2^-15 stay representable
+constexpr float kRescaleThresholdF8 = 2.0f;  // so that 2^6 P <= 2^8 < 448 with a stale max
+
+template <int HD, int EB>
+__device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, const CUtensorMap& tm_k, const CUtensorMap& tm_v,
+                                                    const CUtensorMap& tm_kg, const CUtensorMap& tm_vg, const AttnParams& p,
+                                                    const F8Scales* f8) {
+  using S = Smem<HD, EB>;
+  constexpr bool kF8 = (EB == 1);
   extern __shared__ __align__(1024) uint8_t smem_raw[];    // the only shared memory of the kernel: starts 1024-aligned
   const uint32_t sbase = smem_u32(smem_raw);
   uint8_t* sgen = smem_raw;
@@ -205,8 +218,9 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   auto bar = [&](int i) -> uint32_t { return bar0 + i * 8; };
   volatile int32_t* info = reinterpret_cast<volatile int32_t*>(sgen + S::kInfoOff);
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;   // warp-uniform role id
-  constexpr uint32_t idesc_qk = umma_idesc_bf16(kBM, kBN, 0, 0);
-  constexpr uint32_t idesc_pv = umma_idesc_bf16(kBM, HD, 0, 1);
+  constexpr uint32_t idesc_qk = kF8 ? umma_idesc_e4m3(kBM, kBN, 0, 0) : umma_idesc_bf16(kBM, kBN, 0, 0);
+  constexpr uint32_t idesc_pv = kF8 ? umma_idesc_e4m3(kBM, HD, 0, 1) : umma_idesc_bf16(kBM, HD, 0, 1);
+  constexpr int kPvSteps = kBN * EB / 32;     // MMA K-steps of one P V (16 bf16 keys or 32 e4m3 keys each)
 
   if (warp == 0 && lane == 0) {
     mbar_init(bar(S::bQFull), 1);
@@ -277,7 +291,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         for (int q = 0; q < kNQ; ++q)
 #pragma unroll
           for (int hf = 0; hf < S::kHalves; ++hf)
-            tma_load_2d(q_smem + q * S::kTileBytes + hf * (kBM * 128), &tm_q, bar(S::bQFull), it.h * HD + hf * 64,
+            tma_load_2d(q_smem + q * S::kTileBytes + hf * (kBM * 128), &tm_q, bar(S::bQFull), it.h * HD + hf * S::kHalfElems,
                         it.row0[q]);
       }
       __syncwarp();
@@ -325,11 +339,11 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
           }
           if (gather) {
             if (g_on)
-              tma_gather4(dst + (g >> 5) * (kBN * 128) + (g & 31) * 512, tm_gath, full, it.kvh * HD + (g >> 5) * 64, r.x, r.y, r.z, r.w);
+              tma_gather4(dst + (g >> 5) * (kBN * 128) + (g & 31) * 512, tm_gath, full, it.kvh * HD + (g >> 5) * S::kHalfElems, r.x, r.y, r.z, r.w);
           } else if (ptid == 0) {
 #pragma unroll
             for (int hf = 0; hf < S::kHalves; ++hf)
-              tma_load_2d(dst + hf * (kBN * 128), tm_tile, full, it.kvh * HD + hf * 64, src);
+              tma_load_2d(dst + hf * (kBN * 128), tm_tile, full, it.kvh * HD + hf * S::kHalfElems, src);
           }
         }
         if (++st == (uint32_t)n_stages) { st = 0; ph ^= 1; }
@@ -413,7 +427,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       // MMA operand is built from uniform counters (kst, vst, j) and constants.
 #define SIFT_ISSUE_PV(q, ACC, K0, K1, LAST)                                                                      \
   if (elect_one()) {                                                                                             \
-    issue_pv<HD, q, ACC, K0, K1>(tz, vt, idesc_pv);                                                              \
+    issue_pv<EB, q, ACC, K0, K1>(tz, vt, idesc_pv);                                                              \
     if (LAST) umma_commit(bar(S::bODone + q));                                                                   \
   }                                                                                                              \
   __syncwarp();
@@ -423,9 +437,9 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     mbar_wait(bar(S::bPFull + PART * kNQ + q), pph[q], 202);                                                     \
     tc_fence_after();                                                                                            \
     if (PART == 0 && (fresh & (1 << q))) {                                                                       \
-      SIFT_ISSUE_PV(q, 0, PART * (kBN / 16 / kPvParts), (PART + 1) * (kBN / 16 / kPvParts), PART == kPvParts - 1) \
+      SIFT_ISSUE_PV(q, 0, PART * (kPvSteps / kPvParts), (PART + 1) * (kPvSteps / kPvParts), PART == kPvParts - 1) \
     } else {                                                                                                     \
-      SIFT_ISSUE_PV(q, 1, PART * (kBN / 16 / kPvParts), (PART + 1) * (kBN / 16 / kPvParts), PART == kPvParts - 1) \
+      SIFT_ISSUE_PV(q, 1, PART * (kPvSteps / kPvParts), (PART + 1) * (kPvSteps / kPvParts), PART == kPvParts - 1) \
     }                                                                                                            \
   }
 #define SIFT_PV_STEP(q)                                                                                          \
@@ -438,7 +452,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   SIFT_PV_STEP(q)                                                                                                \
   if (act & (1 << q)) {                                                                                          \
     if (elect_one()) {                                                                                           \
-      issue_qk<HD, q>(tz, q_smem + q * S::kTileBytes, kt, idesc_qk);                                             \
+      issue_qk<HD, EB, q>(tz, q_smem + q * S::kTileBytes, kt, idesc_qk);                                         \
       umma_commit(bar(S::bSFull + q));                                                                           \
     }                                                                                                            \
     __syncwarp();                                                                                                \
@@ -491,7 +505,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
     const uint32_t s_addr = lane_addr + q * 128;
     const uint32_t o_addr = lane_addr + 256 + q * 128;
-    const float sl = p.scale_log2;
+    float sl = p.scale_log2;                 // (e4m3: per q-head, set with the item)
     const int tile_lim = min(kBN, p.tile);
     uint32_t sph = 0;
     uint32_t pv_cnt = 0;
@@ -520,6 +534,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         lim = it.is_dense ? row0 - it.kbase + r + 1 : it.cp - it.c0;
         if (it.is_dense) ngroups = nsteps;                // "frontier" steps: all of them
         paged_item = p.paged && !it.is_dense;
+        if constexpr (kF8) sl = f8->qk_log2[h];
       }
       float m = -INFINITY, l = 0.f;
       for (int e = 0; e < nsteps; ++e, lim -= kBN) {
@@ -554,7 +569,7 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         }
         const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
         const float m_new = fmaxf(m, mx);
-        const bool need = (m_new - m) * sl > kRescaleThreshold;   // (-inf) - (-inf) = NaN -> false
+        const bool need = (m_new - m) * sl > (kF8 ? kRescaleThresholdF8 : kRescaleThreshold);   // (-inf) - (-inf) = NaN -> false
         if (__any_sync(0xffffffffu, need)) {
           const float alpha = need ? ex2((m - m_new) * sl) : 1.f;
           l *= alpha;
@@ -579,20 +594,39 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         const float2 sl2 = make_float2(sl, sl), nm2 = make_float2(neg_m, neg_m);
 #pragma unroll
         for (int c = 0; c < kBN / 32; ++c) {
-          uint32_t pk[16];
+          if constexpr (!kF8) {
+            uint32_t pk[16];
 #pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            const float2 x = fma2(make_float2(s[c * 32 + 2 * i], s[c * 32 + 2 * i + 1]), sl2, nm2);
-            const float2 pr = make_float2(ex2(x.x), ex2(x.y));
-            if (i & 1) sum_b = add2(sum_b, pr); else sum_a = add2(sum_a, pr);
-            pk[i] = pack_bf16x2(pr.x, pr.y);
+            for (int i = 0; i < 16; ++i) {
+              const float2 x = fma2(make_float2(s[c * 32 + 2 * i], s[c * 32 + 2 * i + 1]), sl2, nm2);
+              const float2 pr = make_float2(ex2(x.x), ex2(x.y));
+              if (i & 1) sum_b = add2(sum_b, pr); else sum_a = add2(sum_a, pr);
+              pk[i] = pack_bf16x2(pr.x, pr.y);
+            }
+            // P (bf16) overwrites the first 64 columns of S: 16 packed columns per 32 keys
+            asm volatile(
+                "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                ::"r"(s_addr + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
+                  "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
+                  "r"(pk[15]) : "memory");
+          } else {
+            // e4m3: P is stored as 2^6 P (kP8Shift; the row sum keeps the fp32 P), 8 packed columns per 32 keys
+            uint32_t pk[8];
+            const float2 sh2 = make_float2(kP8Shift, kP8Shift), z2 = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const float2 xa = fma2(make_float2(s[c * 32 + 4 * i], s[c * 32 + 4 * i + 1]), sl2, nm2);
+              const float2 xb = fma2(make_float2(s[c * 32 + 4 * i + 2], s[c * 32 + 4 * i + 3]), sl2, nm2);
+              const float2 pa = make_float2(ex2(xa.x), ex2(xa.y)), pb = make_float2(ex2(xb.x), ex2(xb.y));
+              sum_a = add2(sum_a, pa); sum_b = add2(sum_b, pb);
+              const float2 qa = fma2(pa, sh2, z2), qb = fma2(pb, sh2, z2);
+              pk[i] = pack_e4m3x4(qa.x, qa.y, qb.x, qb.y);
+            }
+            asm volatile(
+                "tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                ::"r"(s_addr + c * 8), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
+                  "r"(pk[7]) : "memory");
           }
-          // P (bf16) overwrites the first 64 columns of S: 16 packed columns per 32 keys
-          asm volatile(
-              "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-              ::"r"(s_addr + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
-                "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
-                "r"(pk[15]) : "memory");
           if ((c + 1) % (4 / kPvParts) == 0 && c != kBN / 32 - 1) {   // a key range is done: let its part of P V start
             tmem_wait_st();
             tc_fence_before();
@@ -614,7 +648,8 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
       if (nsteps > 0) {
         mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 303);
         tc_fence_after();
-        const float inv = (m > -INFINITY) ? 1.f / l : 0.f;   // a row with no allowed key keeps m = -inf (A13)
+        float inv = (m > -INFINITY) ? 1.f / l : 0.f;   // a row with no allowed key keeps m = -inf (A13)
+        if constexpr (kF8) inv *= f8->v[h] * (1.f / kP8Shift);
 #pragma unroll
         for (int c = 0; c < HD / 32; ++c) {
           uint32_t o[32];
@@ -650,6 +685,22 @@ sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
   if (warp == 2) tmem_dealloc(tmem_base, kTmemCols);
 }
 
+template <int HD>
+__global__ void __launch_bounds__(kNumThreads, 1)
+sift_attention_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                      const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_kg,
+                      const __grid_constant__ CUtensorMap tm_vg, const AttnParams p) {
+  sift_attention_body<HD, 2>(tm_q, tm_k, tm_v, tm_kg, tm_vg, p, nullptr);
+}
+
+// e4m3 Q/K/V (head_dim 128): the same body with kind::f8f6f4 MMAs, e4m3 P and per-head scales
+__global__ void __launch_bounds__(kNumThreads, 1)
+sift_attention_f8_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                         const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_kg,
+                         const __grid_constant__ CUtensorMap tm_vg, const AttnParams p, const __grid_constant__ F8Scales f8) {
+  sift_attention_body<128, 1>(tm_q, tm_k, tm_v, tm_kg, tm_vg, p, &f8);
+}
+
 
 // ------------------------------------------------------------------------------------------------
 // host side
@@ -661,32 +712,34 @@ constexpr int kDenseCounterRing = 1024;
 __device__ int32_t g_dense_counters[kDenseCounterRing][2];
 static std::atomic<uint32_t> g_dense_ticket{0};
 
-static int check_tensor(const void* ptr, int64_t stride, const char* name) {
+static int check_tensor(const void* ptr, int64_t stride, const char* name, int elem_bytes = 2) {
   if (!ptr) return set_error(SIFT_ERR_INVALID_ARG, "%s is NULL", name);
-  if (((uintptr_t)ptr & 15) != 0 || (stride * 2) % 16 != 0)
+  if (((uintptr_t)ptr & 15) != 0 || (stride * elem_bytes) % 16 != 0)
     return set_error(SIFT_ERR_INVALID_ARG, "%s base / row stride not 16-byte aligned", name);
   return SIFT_OK;
 }
 
-template <int HD>
+template <int HD, int EB = 2>
 static int launch_attention(AttnParams& p, const void* Q, const void* K, const void* V, int64_t qs, int64_t ks, int64_t vs,
-                            cudaStream_t st) {
+                            cudaStream_t st, const F8Scales* f8 = nullptr) {
   CUtensorMap tq, tk, tv, tkg, tvg;
   int rc;
   const int64_t n = p.n_tokens;
-  if ((rc = make_tensor_map_2d(&tq, Q, n, (int64_t)p.n_q_heads * HD, qs, kBM))) return rc;
-  if ((rc = make_tensor_map_2d(&tk, K, n, (int64_t)p.n_kv_heads * HD, ks, kBN))) return rc;
-  if ((rc = make_tensor_map_2d(&tv, V, n, (int64_t)p.n_kv_heads * HD, vs, kBN))) return rc;
-  if ((rc = make_tensor_map_2d(&tkg, K, n, (int64_t)p.n_kv_heads * HD, ks, 1))) return rc;
-  if ((rc = make_tensor_map_2d(&tvg, V, n, (int64_t)p.n_kv_heads * HD, vs, 1))) return rc;
+  if ((rc = make_tensor_map_2d(&tq, Q, n, (int64_t)p.n_q_heads * HD, qs, kBM, EB))) return rc;
+  if ((rc = make_tensor_map_2d(&tk, K, n, (int64_t)p.n_kv_heads * HD, ks, kBN, EB))) return rc;
+  if ((rc = make_tensor_map_2d(&tv, V, n, (int64_t)p.n_kv_heads * HD, vs, kBN, EB))) return rc;
+  if ((rc = make_tensor_map_2d(&tkg, K, n, (int64_t)p.n_kv_heads * HD, ks, 1, EB))) return rc;
+  if ((rc = make_tensor_map_2d(&tvg, V, n, (int64_t)p.n_kv_heads * HD, vs, 1, EB))) return rc;
   int num_sms = 0;
   if ((rc = device_sm_count(&num_sms))) return rc;
-  if ((rc = ensure_dynamic_smem(reinterpret_cast<const void*>(&sift_attention_kernel<HD>), Smem<HD>::kBytes,
-                                HD == 128 ? kSmemSlotAttn128 : kSmemSlotAttn64)))
+  const void* fn = EB == 1 ? reinterpret_cast<const void*>(&sift_attention_f8_kernel)
+                           : reinterpret_cast<const void*>(&sift_attention_kernel<HD>);
+  if ((rc = ensure_dynamic_smem(fn, Smem<HD, EB>::kBytes, EB == 1 ? kSmemSlotAttnF8 : (HD == 128 ? kSmemSlotAttn128 : kSmemSlotAttn64))))
     return rc;
   const int grid = p.n_items < num_sms ? (p.n_items > 0 ? p.n_items : 1) : num_sms;
   cudaGetLastError();
-  sift_attention_kernel<HD><<<grid, kNumThreads, Smem<HD>::kBytes, st>>>(tq, tk, tv, tkg, tvg, p);
+  if constexpr (EB == 1) sift_attention_f8_kernel<<<grid, kNumThreads, Smem<HD, EB>::kBytes, st>>>(tq, tk, tv, tkg, tvg, p, *f8);
+  else sift_attention_kernel<HD><<<grid, kNumThreads, Smem<HD>::kBytes, st>>>(tq, tk, tv, tkg, tvg, p);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "attention launch: %s", cudaGetErrorString(e));
   count_launch(1);
@@ -697,25 +750,20 @@ static int launch_attention(AttnParams& p, const void* Q, const void* K, const v
 
 using namespace sift;
 
-extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, const void* Q, const void* K, const void* V,
-                                      int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
-                                      const void* metadata, void* O, int64_t o_row_stride, float* lse,
-                                      float softmax_scale, void* stream) {
+// arguments common to the bf16 and the e4m3 entry: metadata pointers of the layer, output, scale
+static int sparse_params(const sift_shape* shape, int32_t layer, const void* metadata, void* O, int64_t o_row_stride, float* lse,
+                         float softmax_scale, AttnParams* pp) {
   sift_md_layout lay;
   int rc = compute_layout(shape, &lay);
   if (rc) return rc;
   if (layer < 0 || layer >= shape->n_layers) return set_error(SIFT_ERR_INVALID_ARG, "layer %d out of range", layer);
   if (!metadata) return set_error(SIFT_ERR_INVALID_ARG, "metadata is NULL");
-  if ((rc = check_tensor(Q, q_row_stride, "Q")) || (rc = check_tensor(K, k_row_stride, "K")) ||
-      (rc = check_tensor(V, v_row_stride, "V")) || (rc = check_tensor(O, o_row_stride, "O")))
-    return rc;
+  if ((rc = check_tensor(O, o_row_stride, "O"))) return rc;
   const int Hq = shape->n_q_heads, D = shape->n_docs, HD = shape->head_dim;
-  if (q_row_stride < (int64_t)Hq * HD || o_row_stride < (int64_t)Hq * HD || k_row_stride < (int64_t)shape->n_kv_heads * HD ||
-      v_row_stride < (int64_t)shape->n_kv_heads * HD)
-    return set_error(SIFT_ERR_INVALID_ARG, "row stride smaller than heads*head_dim");
+  if (o_row_stride < (int64_t)Hq * HD) return set_error(SIFT_ERR_INVALID_ARG, "row stride smaller than heads*head_dim");
   const char* b = static_cast<const char*>(metadata);
   auto at = [&](size_t off) { return reinterpret_cast<const int32_t*>(b + off); };
-  AttnParams p;
+  AttnParams& p = *pp;
   memset(&p, 0, sizeof(p));
   const int64_t lh0 = (int64_t)layer * Hq;
   p.tile_seg = at(lay.tile_seg); p.tile_row0 = at(lay.tile_row0); p.tile_rows = at(lay.tile_rows);
@@ -737,8 +785,52 @@ extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, co
   p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
   const float sc = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf((float)HD);
   p.scale_log2 = sc * 1.4426950408889634f;
+  return SIFT_OK;
+}
+
+extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, const void* Q, const void* K, const void* V,
+                                      int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
+                                      const void* metadata, void* O, int64_t o_row_stride, float* lse,
+                                      float softmax_scale, void* stream) {
+  AttnParams p;
+  int rc = sparse_params(shape, layer, metadata, O, o_row_stride, lse, softmax_scale, &p);
+  if (rc) return rc;
+  if ((rc = check_tensor(Q, q_row_stride, "Q")) || (rc = check_tensor(K, k_row_stride, "K")) ||
+      (rc = check_tensor(V, v_row_stride, "V")))
+    return rc;
+  const int Hq = shape->n_q_heads, HD = shape->head_dim;
+  if (q_row_stride < (int64_t)Hq * HD || k_row_stride < (int64_t)shape->n_kv_heads * HD ||
+      v_row_stride < (int64_t)shape->n_kv_heads * HD)
+    return set_error(SIFT_ERR_INVALID_ARG, "row stride smaller than heads*head_dim");
   if (HD == 128) return launch_attention<128>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
   return launch_attention<64>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
+}
+
+extern "C" int sift_prefill_attention_fp8(const sift_shape* shape, int32_t layer, const void* Q8, const void* K8, const void* V8,
+                                          int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
+                                          const float* q_scale, const float* k_scale, const float* v_scale,
+                                          const void* metadata, void* O, int64_t o_row_stride, float* lse,
+                                          float softmax_scale, void* stream) {
+  AttnParams p;
+  int rc = sparse_params(shape, layer, metadata, O, o_row_stride, lse, softmax_scale, &p);
+  if (rc) return rc;
+  if (shape->head_dim != 128) return set_error(SIFT_ERR_UNSUPPORTED, "e4m3 Q/K/V: head_dim %d (128 supported)", shape->head_dim);
+  if ((rc = check_tensor(Q8, q_row_stride, "Q8", 1)) || (rc = check_tensor(K8, k_row_stride, "K8", 1)) ||
+      (rc = check_tensor(V8, v_row_stride, "V8", 1)))
+    return rc;
+  if (!q_scale || !k_scale || !v_scale) return set_error(SIFT_ERR_INVALID_ARG, "scale array is NULL");
+  const int Hq = shape->n_q_heads, Hkv = shape->n_kv_heads, HD = 128;
+  if (q_row_stride < (int64_t)Hq * HD || k_row_stride < (int64_t)Hkv * HD || v_row_stride < (int64_t)Hkv * HD)
+    return set_error(SIFT_ERR_INVALID_ARG, "row stride smaller than heads*head_dim");
+  static thread_local F8Scales f8;
+  for (int h = 0; h < Hq; ++h) {
+    const int g = h / (Hq / Hkv);
+    if (!(q_scale[h] > 0.f) || !(k_scale[g] > 0.f) || !(v_scale[g] > 0.f))
+      return set_error(SIFT_ERR_INVALID_ARG, "scales must be positive (q-head %d)", h);
+    f8.qk_log2[h] = p.scale_log2 * q_scale[h] * k_scale[g];
+    f8.v[h] = v_scale[g];
+  }
+  return launch_attention<128, 1>(p, Q8, K8, V8, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream, &f8);
 }
 
 extern "C" int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,

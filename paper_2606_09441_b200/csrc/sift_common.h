@@ -43,9 +43,11 @@ void count_launch(int n = 1);
 int launch_decode(const sift_shape* s, const sift_md_layout& lay, const DocTable& dt,
                   const uint8_t* la_base, const uint8_t* ca_base, void* md, cudaStream_t st);
 
-// 2-D bf16 tensor [rows][cols] with a row stride of `row_stride` elements; box = 64 columns x box_rows, 128-byte swizzle
-// (the image tcgen05's SWIZZLE_128B descriptors read).  Shared by the attention and the encoder launchers.
-int make_tensor_map_2d(CUtensorMap* m, const void* base, int64_t rows, int64_t cols, int64_t row_stride, int box_rows);
+// 2-D tensor [rows][cols] of bf16 (elem_bytes 2) or bytes (1: e4m3) with a row stride of `row_stride` elements; box = 128
+// bytes of a row x box_rows, 128-byte swizzle (the image tcgen05's SWIZZLE_128B descriptors read).  Shared by the
+// attention and the encoder launchers.
+int make_tensor_map_2d(CUtensorMap* m, const void* base, int64_t rows, int64_t cols, int64_t row_stride, int box_rows,
+                       int elem_bytes = 2);
 // SM count of the current device, and the once-per-(device, kernel) opt-in to `bytes` of dynamic shared memory.
 // `slot` numbers the kernels of the library (kSmemSlot*): cudaFuncSetAttribute is a per-device attribute.
 int device_sm_count(int* num_sms);

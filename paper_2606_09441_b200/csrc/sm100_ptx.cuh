@@ -126,19 +126,34 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
 // Same two forms with the TMEM addresses given as (uniform run-time base) + (compile-time offset): the adds sit next
 // to the MMA, so the addresses are rebuilt in uniform registers instead of being hoisted into vector registers and
 // moved back with R2UR on every issue.
-template <uint32_t DOFF>
+// F8 = false: kind::f16 (bf16 operands); F8 = true: kind::f8f6f4 (e4m3 operands, 32 elements per K step)
+template <uint32_t DOFF, bool F8 = false>
 __device__ __forceinline__ void umma_ss_off(uint32_t tbase, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t.reg .b32 d;\n\tsetp.ne.b32 p, %4, 0;\n\tadd.u32 d, %0, %5;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [d], %1, %2, %3, p;\n\t}"
-      ::"r"(tbase), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accum), "n"(DOFF) : "memory");
+  if constexpr (F8) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b32 d;\n\tsetp.ne.b32 p, %4, 0;\n\tadd.u32 d, %0, %5;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f8f6f4 [d], %1, %2, %3, p;\n\t}"
+        ::"r"(tbase), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accum), "n"(DOFF) : "memory");
+  } else {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b32 d;\n\tsetp.ne.b32 p, %4, 0;\n\tadd.u32 d, %0, %5;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [d], %1, %2, %3, p;\n\t}"
+        ::"r"(tbase), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accum), "n"(DOFF) : "memory");
+  }
 }
-template <uint32_t DOFF, uint32_t AOFF>
+template <uint32_t DOFF, uint32_t AOFF, bool F8 = false>
 __device__ __forceinline__ void umma_ts_off(uint32_t tbase, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t.reg .b32 d, a;\n\tsetp.ne.b32 p, %3, 0;\n\tadd.u32 d, %0, %4;\n\tadd.u32 a, %0, %5;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [d], [a], %1, %2, p;\n\t}"
-      ::"r"(tbase), "l"(b_desc), "r"(idesc), "r"(accum), "n"(DOFF), "n"(AOFF) : "memory");
+  if constexpr (F8) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b32 d, a;\n\tsetp.ne.b32 p, %3, 0;\n\tadd.u32 d, %0, %4;\n\tadd.u32 a, %0, %5;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f8f6f4 [d], [a], %1, %2, p;\n\t}"
+        ::"r"(tbase), "l"(b_desc), "r"(idesc), "r"(accum), "n"(DOFF), "n"(AOFF) : "memory");
+  } else {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b32 d, a;\n\tsetp.ne.b32 p, %3, 0;\n\tadd.u32 d, %0, %4;\n\tadd.u32 a, %0, %5;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [d], [a], %1, %2, p;\n\t}"
+        ::"r"(tbase), "l"(b_desc), "r"(idesc), "r"(accum), "n"(DOFF), "n"(AOFF) : "memory");
+  }
 }
 
 // Shared-memory matrix descriptor, 128-byte swizzle.  K-major: rows of 64 bf16 (128 B), 8-row groups SBO apart.
@@ -156,6 +171,12 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo
 __host__ __device__ constexpr uint32_t umma_idesc_bf16(int m, int n, int a_mn_major, int b_mn_major) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn_major << 15) | ((uint32_t)b_mn_major << 16) |
          ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+
+// kind::f8f6f4 instruction descriptor: e4m3 x e4m3 -> fp32 (a_format = b_format = 0 = E4M3; MN-major is valid for E4M3)
+__host__ __device__ constexpr uint32_t umma_idesc_e4m3(int m, int n, int a_mn_major, int b_mn_major) {
+  return (1u << 4) | ((uint32_t)a_mn_major << 15) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(n >> 3) << 17) |
+         ((uint32_t)(m >> 4) << 24);
 }
 
 // TMEM <-> registers, one row (lane) per thread, 32 consecutive 32-bit columns
@@ -185,6 +206,13 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
 }
+// four floats -> four e4m3 bytes, p0 in the lowest byte (satfinite: 448 is the largest magnitude)
+__device__ __forceinline__ uint32_t pack_e4m3x4(float p0, float p1, float p2, float p3) {
+  uint32_t r;
+  asm("{\n\t.reg .b16 lo, hi;\n\tcvt.rn.satfinite.e4m3x2.f32 lo, %2, %1;\n\tcvt.rn.satfinite.e4m3x2.f32 hi, %4, %3;\n\t"
+      "mov.b32 %0, {lo, hi};\n\t}" : "=r"(r) : "f"(p0), "f"(p1), "f"(p2), "f"(p3));
+  return r;
+}
 __device__ __forceinline__ float ex2(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -212,24 +240,5 @@ __device__ __forceinline__ float2 add2(float2 a, float2 b) {
   asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
   return d;
 }
-// 2^x for a pair on the FMA/ALU pipes instead of the MUFU: round-to-nearest split x = n + f (magic-number add),
-// cubic minimax polynomial for 2^f on [-0.5, 0.5] (max relative error 7.5e-5, far below the bf16 rounding of P),
-// exponent patched in with an integer add.  x is clamped at -126 (masked entries are -inf -> ~1e-38 ~ 0).
-__device__ __forceinline__ float2 ex2_poly2(float2 x) {
-  x.x = fmaxf(x.x, -126.f);
-  x.y = fmaxf(x.y, -126.f);
-  const float kMagic = 12582912.f;   // 1.5 * 2^23
-  const float2 t = add2(x, make_float2(kMagic, kMagic));
-  const float2 n = add2(t, make_float2(-kMagic, -kMagic));
-  const float2 f = fma2(n, make_float2(-1.f, -1.f), x);
-  float2 p = fma2(f, make_float2(0.05517132207751274f, 0.05517132207751274f), make_float2(0.24261054396629333f, 0.24261054396629333f));
-  p = fma2(p, f, make_float2(0.6932609677314758f, 0.6932609677314758f));
-  p = fma2(p, f, make_float2(0.9999281167984009f, 0.9999281167984009f));
-  float2 r;
-  r.x = __int_as_float(__float_as_int(p.x) + (__float_as_int(t.x) << 23));
-  r.y = __int_as_float(__float_as_int(p.y) + (__float_as_int(t.y) << 23));
-  return r;
-}
-
 }  // namespace ptx
 }  // namespace sift

@@ -17,7 +17,7 @@ def _built():
 
 def test_exports_match_header():
     hdr = open(build.ROOT + "/include/sift.h").read()
-    declared = set(re.findall(r"\b(sift_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(sift_[a-z0-9_]+)\s*\(", hdr))
     declared -= {"sift_status"}
     assert declared == set(api.EXPORTS), declared ^ set(api.EXPORTS)
     L = C.CDLL(build.LIB)
