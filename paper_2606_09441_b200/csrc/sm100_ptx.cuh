@@ -43,16 +43,29 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
       : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
   return ok != 0;
 }
-// Bounded wait: a protocol bug traps (with the barrier id) instead of hanging the GPU box.
+// Bounded wait: a protocol bug traps instead of hanging the GPU box.  The bound is TIME (10 s of %globaltimer, looked
+// at every 2^16 failed polls), not a poll count: a legitimately long stall (a debugger, a sanitizer, a co-resident kernel
+// holding TMEM) does not kill the context.  Before trapping, the wait site's tag is left in g_barrier_timeout_tag (readable
+// with cudaMemcpyFromSymbol from a fresh context / cuda-gdb).
+static __device__ int g_barrier_timeout_tag;
+static __device__ __noinline__ void mbar_timeout(int tag, uint32_t parity) {
+  g_barrier_timeout_tag = tag;
+  __threadfence_system();
+#ifdef SIFT_DEBUG_BARRIERS
+  printf("sift: mbarrier timeout tag=%d block=%d thread=%d parity=%u\n", tag, (int)blockIdx.x, (int)threadIdx.x, parity);
+#endif
+  __trap();
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int tag = 0) {
   if (mbar_try_wait(bar, parity)) return;
   uint32_t spins = 0;
+  uint64_t t0 = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if (++spins > (1u << 24)) {
-#ifdef SIFT_DEBUG_BARRIERS   // the message costs a printf frame at every wait site (registers, code size): debug builds only
-      printf("sift: mbarrier timeout tag=%d block=%d thread=%d parity=%u\n", tag, (int)blockIdx.x, (int)threadIdx.x, parity);
-#endif
-      __trap();
+    if ((++spins & 0xFFFFu) == 0) {
+      uint64_t now;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > 10000000000ull) mbar_timeout(tag, parity);
     }
   }
 }
