@@ -561,41 +561,22 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
 #pragma unroll
           for (int c = 0; c < kBN; ++c) s[c] = (c < cur_lim) ? s[c] : -INFINITY;
         }
-        float mx4[4] = {s[0], s[1], s[2], s[3]};                  // four independent chains
+        // row max: four independent chains of 3-input max
+        auto max32 = [&](int c0_) {
+          float a0 = s[c0_], a1 = s[c0_ + 1], a2 = s[c0_ + 2], a3 = s[c0_ + 3];
 #pragma unroll
-        for (int c = 4; c < kBN; c += 4) {
-          mx4[0] = fmaxf(mx4[0], s[c]); mx4[1] = fmaxf(mx4[1], s[c + 1]);
-          mx4[2] = fmaxf(mx4[2], s[c + 2]); mx4[3] = fmaxf(mx4[3], s[c + 3]);
-        }
-        const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3]));
-        const float m_new = fmaxf(m, mx);
-        const bool need = (m_new - m) * sl > (kF8 ? kRescaleThresholdF8 : kRescaleThreshold);   // (-inf) - (-inf) = NaN -> false
-        if (__any_sync(0xffffffffu, need)) {
-          const float alpha = need ? ex2((m - m_new) * sl) : 1.f;
-          l *= alpha;
-          if (need) m = m_new;
-          if (e > 0) {
-            // O of this tile must hold every P*V issued so far before it is rescaled
-            mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 302);
-            tc_fence_after();
-#pragma unroll
-            for (int c = 0; c < HD / 32; ++c) {
-              uint32_t o[32];
-              tmem_ld32(o_addr + c * 32, o);
-              tmem_wait_ld();
-#pragma unroll
-              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-              tmem_st32(o_addr + c * 32, o);
-            }
+          for (int c = 4; c < 32; c += 4) {
+            a0 = fmaxf(a0, s[c0_ + c]); a1 = fmaxf(a1, s[c0_ + c + 1]);
+            a2 = fmaxf(a2, s[c0_ + c + 2]); a3 = fmaxf(a3, s[c0_ + c + 3]);
           }
-        }
-        const float neg_m = (m == -INFINITY) ? 0.f : -m * sl;
-        float2 sum_a = make_float2(0.f, 0.f), sum_b = make_float2(0.f, 0.f);
-        const float2 sl2 = make_float2(sl, sl), nm2 = make_float2(neg_m, neg_m);
-#pragma unroll
-        for (int c = 0; c < kBN / 32; ++c) {
+          return fmaxf(fmaxf(a0, a1), fmaxf(a2, a3));
+        };
+        constexpr float kThr = kF8 ? kRescaleThresholdF8 : kRescaleThreshold;
+        float2 sum_a, sum_b;
+        // exponentials of 32 columns -> packed P in pk (bf16: 16 words, e4m3: 8 words, stored as 2^6 P)
+        auto exp_chunk = [&](int c, uint32_t* pk, float neg_m) {
+          const float2 sl2 = make_float2(sl, sl), nm2 = make_float2(neg_m, neg_m);
           if constexpr (!kF8) {
-            uint32_t pk[16];
 #pragma unroll
             for (int i = 0; i < 16; ++i) {
               const float2 x = fma2(make_float2(s[c * 32 + 2 * i], s[c * 32 + 2 * i + 1]), sl2, nm2);
@@ -603,15 +584,7 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
               if (i & 1) sum_b = add2(sum_b, pr); else sum_a = add2(sum_a, pr);
               pk[i] = pack_bf16x2(pr.x, pr.y);
             }
-            // P (bf16) overwrites the first 64 columns of S: 16 packed columns per 32 keys
-            asm volatile(
-                "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-                ::"r"(s_addr + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
-                  "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
-                  "r"(pk[15]) : "memory");
           } else {
-            // e4m3: P is stored as 2^6 P (kP8Shift; the row sum keeps the fp32 P), 8 packed columns per 32 keys
-            uint32_t pk[8];
             const float2 sh2 = make_float2(kP8Shift, kP8Shift), z2 = make_float2(0.f, 0.f);
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
@@ -622,16 +595,60 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
               const float2 qa = fma2(pa, sh2, z2), qb = fma2(pb, sh2, z2);
               pk[i] = pack_e4m3x4(qa.x, qa.y, qb.x, qb.y);
             }
+          }
+        };
+        // P overwrites the first columns of S (bf16: 16 packed columns per 32 keys, e4m3: 8); a finished key range lets
+        // its part of P V start
+        auto store_chunk = [&](int c, const uint32_t* pk) {
+          if constexpr (!kF8) {
+            asm volatile(
+                "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                ::"r"(s_addr + c * 16), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
+                  "r"(pk[7]), "r"(pk[8]), "r"(pk[9]), "r"(pk[10]), "r"(pk[11]), "r"(pk[12]), "r"(pk[13]), "r"(pk[14]),
+                  "r"(pk[15]) : "memory");
+          } else {
             asm volatile(
                 "tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                 ::"r"(s_addr + c * 8), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]), "r"(pk[5]), "r"(pk[6]),
                   "r"(pk[7]) : "memory");
           }
-          if ((c + 1) % (4 / kPvParts) == 0 && c != kBN / 32 - 1) {   // a key range is done: let its part of P V start
+          if ((c + 1) % (4 / kPvParts) == 0 && c != kBN / 32 - 1) {
             tmem_wait_st();
             tc_fence_before();
             mbar_arrive(bar(S::bPFull + ((c + 1) / (4 / kPvParts) - 1) * kNQ + q));
           }
+        };
+        {
+          const float mx = fmaxf(fmaxf(max32(0), max32(32)), fmaxf(max32(64), max32(96)));
+          const float m_new = fmaxf(m, mx);
+          const bool need = (m_new - m) * sl > kThr;   // (-inf) - (-inf) = NaN -> false
+          if (__any_sync(0xffffffffu, need)) {
+            const float alpha = need ? ex2((m - m_new) * sl) : 1.f;
+            l *= alpha;
+            if (need) m = m_new;
+            if (e > 0) {
+              // O of this tile must hold every P*V issued so far before it is rescaled
+              mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 302);
+              tc_fence_after();
+#pragma unroll
+              for (int c = 0; c < HD / 32; ++c) {
+                uint32_t o[32];
+                tmem_ld32(o_addr + c * 32, o);
+                tmem_wait_ld();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                tmem_st32(o_addr + c * 32, o);
+              }
+            }
+          }
+        }
+        const float neg_m = (m == -INFINITY) ? 0.f : -m * sl;
+        sum_a = make_float2(0.f, 0.f); sum_b = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int c = 0; c < kBN / 32; ++c) {
+          uint32_t pk[kF8 ? 8 : 16];
+          exp_chunk(c, pk, neg_m);
+          store_chunk(c, pk);
         }
         const float2 sum2 = add2(sum_a, sum_b);
         const float sum0 = sum2.x, sum1 = sum2.y;
