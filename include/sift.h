@@ -49,7 +49,9 @@ typedef struct {
   uint32_t struct_size; /* = sizeof(sift_shape) */
   int32_t n_layers, n_q_heads, n_kv_heads, head_dim;
   int32_t n_docs, query_len;
-  int32_t tile;       /* T: 64 or 128 (M-block = N-block = T) */
+  int32_t tile;       /* T: 64 or 128 (M-block = N-block = T).  128 is the tuned size; 64 is
+                         functional: a 64-row query tile still occupies a 128-lane accumulator and a 64-key local tile
+                         a 128-key MMA step, so at most half of the tensor work is useful */
   int32_t cross_gran; /* G: 1 = one CA bit per key token (BASELINE.json configs); tile = one bit per page */
   const int32_t* doc_offsets; /* HOST, n_docs + 1 entries */
   /* ---- several prompts in one call (optional; struct_size = SIFT_SHAPE_SIZE_V1 or n_prompts <= 1: one prompt) ----

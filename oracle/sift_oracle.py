@@ -684,12 +684,11 @@ def encode_from_probabilities(p: np.ndarray, tile: int, gran: int, alpha: float,
     hit = (p >= beta) & np.tril(np.ones((n, n), dtype=bool))
     col_hits = hit.sum(axis=0).astype(np.int64)          # per key column
     ca_bits, hits_g, cells_g = [], [], []
-    g32 = float(np.float32(gamma))                       # the library receives gamma as fp32 and decides in fp64
     for g in range(n_groups):
         ks = range(g * gran, min(n, (g + 1) * gran))
         hits = int(sum(int(col_hits[k]) for k in ks))
         cells = int(sum(n - k for k in ks))
-        ca_bits.append(1 if hits > g32 * cells else 0)
+        ca_bits.append(1 if hits > gamma * cells else 0)   # "exceeds gamma" (L209), gamma as given
         hits_g.append(hits)
         cells_g.append(cells)
     info = {"la_bits": np.array(la_bits), "la_max": np.array(la_max), "ca_bits": np.array(ca_bits),

@@ -198,7 +198,7 @@ sift_encode_pack_kernel(const EncParams p, float gamma, uint8_t* la_out, uint8_t
       if (g >= n_groups) break;
       long long hits = 0, cells = 0;
       for (int key = g * G; key < min(L, (g + 1) * G); ++key) { hits += cc[key]; cells += L - key; }
-      // "exceeds gamma", decided in fp64 on the fp32 value of gamma (the oracle does the same)
+      // "exceeds gamma", decided in fp64 on the fp32 value of gamma the ABI carries
       if ((double)hits > (double)gamma * (double)cells) v |= 0x80u >> k;
     }
     ca_out[(int64_t)h * ca_bytes + b] = (uint8_t)v;

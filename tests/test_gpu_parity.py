@@ -214,7 +214,8 @@ def _encode_case(n, hq, hkv, d, tile, gran, seed, alpha=1e-3, beta=1e-2, gamma=0
     n_la, n_ca = pt * (pt + 1) // 2, -(-n // gran)
     checked = skipped = 0
     for h in range(hq):
-        la_o, ca_o, info = so.encode_document(q, k, h, tile, gran, alpha, beta, gamma)
+        # the ABI takes gamma as a float: the oracle is given the value the library sees (the caveat is the test's)
+        la_o, ca_o, info = so.encode_document(q, k, h, tile, gran, alpha, beta, float(np.float32(gamma)))
         assert la.shape[1] == len(la_o) and ca.shape[1] == len(ca_o)
         p = info["p"]
         # padding bits must be zero
