@@ -71,6 +71,7 @@ struct AttnParams {
   int32_t dense;  // 1: every M-block is a DENSE item over n_tokens rows
   int32_t n_tokens, n_q_heads, n_kv_heads, tile;
   int32_t kv_per_group;     // dense comparator: kv heads scheduled together (sched_kv_heads_per_group)
+  int32_t o_vec32;          // O rows are 32-byte aligned: the epilogue may use 256-bit stores
   int32_t paged;            // cross_gran == tile: cross entries are global tile ids, one tiled step each
   __nv_bfloat16* o;
   int64_t o_row_stride;
@@ -101,7 +102,7 @@ struct Smem {
   static constexpr int bItemFull = bODone + kNQ, bItemEmpty = bItemFull + 2;
   static constexpr int kNumBars = bItemEmpty + 2;
   static constexpr int kInfoOff = kBarOff + ((kNumBars * 8 + 15) / 16) * 16;
-  // info words: [0] tmem base, [1..2] item ring, [4 .. 4+kKStages) per-K-stage step info
+  // info words: [0] tmem base, [1..2] item ring, [3] "the item has MMA steps" (item warp -> MMA issuer), [4 .. 4+kKStages) per-K-stage step info
   static constexpr int kBytes = kInfoOff + 64;
   static_assert(kBytes <= 227 * 1024, "shared memory budget");
 };
@@ -204,6 +205,24 @@ struct F8Scales {
 constexpr float kP8Shift = 64.f;             // e4m3 P is stored as 2^6 P: weights down to 2^-15 stay representable
 constexpr float kRescaleThresholdF8 = 2.0f;  // so that 2^6 P <= 2^8 < 448 with a stale max
 
+// N bf16 of one row of O (packed in pairs) to global memory
+template <int HD>
+__device__ __forceinline__ void store_o_row(__nv_bfloat16* row, const uint32_t (&w)[HD / 2], bool vec32) {
+  if (vec32) {
+    // 32-byte stores: every lane fills a whole sector of its own row (a thread owns a row, so a 16-byte store touches
+    // half a sector; +0.7% at 32K, +1.8% at 10K)
+#pragma unroll
+    for (int i = 0; i < HD / 16; ++i)
+      asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(row + i * 16), "r"(w[8 * i]), "r"(w[8 * i + 1]),
+                   "r"(w[8 * i + 2]), "r"(w[8 * i + 3]), "r"(w[8 * i + 4]), "r"(w[8 * i + 5]), "r"(w[8 * i + 6]),
+                   "r"(w[8 * i + 7]) : "memory");
+  } else {
+#pragma unroll
+    for (int i = 0; i < HD / 8; ++i)
+      *reinterpret_cast<uint4*>(row + i * 8) = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+  }
+}
+
 template <int HD, int EB>
 __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, const CUtensorMap& tm_k, const CUtensorMap& tm_v,
                                                     const CUtensorMap& tm_kg, const CUtensorMap& tm_vg, const AttnParams& p,
@@ -286,6 +305,13 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
       // ---- Q tiles
       mbar_wait(bar(S::bQEmpty), (it_n & 1) ^ 1, 101);
       if (lane == 0) {
+        // "this item has MMA steps", for the MMA issuer: it reads the word after its wait on bQFull (this thread's
+        // arrive below releases it), so the issuer never repeats the dependent global loads of load_item, which sat on
+        // its serial path at every item boundary (~3000 clk with the tensor pipe idle)
+        bool hs = it.is_dense || it.cp > it.c0;
+#pragma unroll
+        for (int q = 0; q < kNQ; ++q) hs = hs || it.lcnt[q] > 0;
+        info[3] = hs ? 1 : 0;
         mbar_arrive_expect_tx(bar(S::bQFull), kNQ * S::kTileBytes);
 #pragma unroll
         for (int q = 0; q < kNQ; ++q)
@@ -407,15 +433,8 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
       const int code = __shfl_sync(0xffffffffu, (int)info[1 + slot], 0);
       if (lane == 0) mbar_arrive(bar(S::bItemEmpty + slot));
       if (code < 0) break;
-      int has_steps;
-      {
-        const Item it = load_item(p, code);
-        bool hs = it.is_dense || it.cp > it.c0;
-#pragma unroll
-        for (int q = 0; q < kNQ; ++q) hs = hs || it.lcnt[q] > 0;
-        has_steps = __shfl_sync(0xffffffffu, (int)hs, 0);
-      }
       mbar_wait(bar(S::bQFull), it_n & 1, 201);
+      const int has_steps = __shfl_sync(0xffffffffu, (int)info[3], 0);   // written by the item warp before its Q loads
       if (!has_steps) {
         if (lane == 0) mbar_arrive(bar(S::bQEmpty));
         continue;
@@ -673,15 +692,11 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
           tmem_ld32(o_addr + c * 32, o);
           tmem_wait_ld();
           if (row_ok) {
+            uint32_t w[16];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              uint4 w;
-              w.x = pack_bf16x2(__uint_as_float(o[8 * i + 0]) * inv, __uint_as_float(o[8 * i + 1]) * inv);
-              w.y = pack_bf16x2(__uint_as_float(o[8 * i + 2]) * inv, __uint_as_float(o[8 * i + 3]) * inv);
-              w.z = pack_bf16x2(__uint_as_float(o[8 * i + 4]) * inv, __uint_as_float(o[8 * i + 5]) * inv);
-              w.w = pack_bf16x2(__uint_as_float(o[8 * i + 6]) * inv, __uint_as_float(o[8 * i + 7]) * inv);
-              *reinterpret_cast<uint4*>(orow + c * 32 + i * 8) = w;
-            }
+            for (int i = 0; i < 16; ++i)
+              w[i] = pack_bf16x2(__uint_as_float(o[2 * i]) * inv, __uint_as_float(o[2 * i + 1]) * inv);
+            store_o_row<32>(orow + c * 32, w, p.o_vec32 != 0);
           }
         }
         tc_fence_before();
@@ -800,6 +815,7 @@ static int sparse_params(const sift_shape* shape, int32_t layer, const void* met
   p.n_q_heads = Hq; p.n_kv_heads = shape->n_kv_heads; p.tile = shape->tile;
   p.paged = (shape->cross_gran != 1);
   p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
+  p.o_vec32 = (((uintptr_t)O & 31) == 0 && (o_row_stride * 2) % 32 == 0);
   const float sc = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf((float)HD);
   p.scale_log2 = sc * 1.4426950408889634f;
   return SIFT_OK;
@@ -874,6 +890,7 @@ extern "C" int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, 
   if (cudaMemsetAsync(p.counters, 0, 2 * sizeof(int32_t), (cudaStream_t)stream) != cudaSuccess)
     return set_error(SIFT_ERR_CUDA, "cudaMemsetAsync(dense counters) failed");
   p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
+  p.o_vec32 = (((uintptr_t)O & 31) == 0 && (o_row_stride * 2) % 32 == 0);
   const float sc = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf((float)head_dim);
   p.scale_log2 = sc * 1.4426950408889634f;
   if (head_dim == 128) return launch_attention<128>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
