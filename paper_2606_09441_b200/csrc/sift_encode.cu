@@ -55,7 +55,8 @@ sift_encode_scores_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid
   auto bar = [&](int i) -> uint32_t { return sbase + S::kBarOff + i * 8; };
   volatile int32_t* info = reinterpret_cast<volatile int32_t*>(smem_raw + S::kInfoOff);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int i = blockIdx.x, h = blockIdx.y, kvh = h / (p.n_q_heads / p.n_kv_heads);
+  const int i = (int)gridDim.x - 1 - (int)blockIdx.x;       // longest row blocks (most key blocks) first
+  const int h = blockIdx.y, kvh = h / (p.n_q_heads / p.n_kv_heads);
   const int L = p.doc_len, T = p.tile;
   const int n_j = i + 1;                                   // key blocks 0 .. i (causal)
   constexpr uint32_t idesc = umma_idesc_bf16(128, 128, 0, 0);
@@ -104,6 +105,7 @@ sift_encode_scores_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid
   const int r = tid, row = i * 128 + r;
   const bool row_ok = row < L;
   const float lse2 = row_ok ? p.lse[(int64_t)h * L + row] * 1.4426950408889634f : INFINITY;
+  const float thr_a = (p.log2_alpha + lse2) / p.sl, thr_b = (p.log2_beta + lse2) / p.sl;   // thresholds on the raw score
   const uint32_t lane_addr = (uint32_t)(warp * 32) << 16;
   const int rh = (T == 64) ? (warp >> 1) : 0;              // LA row sub-tile of this warp inside the 128-row block
   const int pt = (L + T - 1) / T;
@@ -123,15 +125,33 @@ sift_encode_scores_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid
       uint32_t raw[32];
       tmem_ld32(tmem + lane_addr + st * 128 + c * 32, raw);
       tmem_wait_ld();
+      // log2 p = s * sl - lse2 >= log2(threshold)  <=>  s >= (log2(threshold) + lse2) / sl: one comparison of the raw
+      // score against a per-row constant (rows beyond the document have lse2 = +inf: never true).  Off the diagonal
+      // every key is causal, and "some p >= alpha" is one comparison of the row's maximum: ~2.5 instructions per score
+      // instead of ~14 (the kernel is bound by these, not by the MMAs).
       uint32_t wb = 0;
-      bool aa = false;
+      bool aa;
+      if (j < i) {
+        float mxs = -INFINITY;
 #pragma unroll
-      for (int cc = 0; cc < 32; ++cc) {
-        const int key = key0 + c * 32 + cc;
-        const float x = fmaf(__uint_as_float(raw[cc]), p.sl, -lse2);     // log2 of the probability
-        const bool valid = key <= row;                                    // causal; row_ok rows only (lse2 = inf otherwise)
-        aa = aa || (valid && x >= p.log2_alpha);
-        wb |= (valid && x >= p.log2_beta) ? (1u << cc) : 0u;
+        for (int cc = 0; cc < 32; ++cc) {
+          const float sc = __uint_as_float(raw[cc]);
+          mxs = fmaxf(mxs, sc);
+          if (sc >= thr_b) wb |= 1u << cc;
+        }
+        aa = mxs >= thr_a;
+      } else {                                                            // diagonal block: keys after the row are not causal
+        uint32_t wa = 0;
+#pragma unroll
+        for (int cc = 0; cc < 32; ++cc) {
+          const float sc = __uint_as_float(raw[cc]);
+          if (sc >= thr_b) wb |= 1u << cc;
+          if (sc >= thr_a) wa |= 1u << cc;
+        }
+        const int lim = row - key0 - c * 32;                              // columns 0 .. lim of this chunk are causal
+        const uint32_t vm = lim >= 31 ? 0xffffffffu : (lim < 0 ? 0u : ((2u << lim) - 1u));
+        wb &= vm;
+        aa = (wa & vm) != 0u;
       }
       any_a[c >> 1] = any_a[c >> 1] || aa;
       // per-key counts of this warp's 32 rows: transpose the 32 x 32 bit matrix (lane = row, bit = column) with five
@@ -146,30 +166,21 @@ sift_encode_scores_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid
       const int cnt = __popc(xt);
       if (cnt) atomicAdd(&p.col_cnt[(int64_t)h * p.len128 + key0 + c * 32 + lane], cnt);
     }
-    if (T == 64) {
-#pragma unroll
-      for (int ch = 0; ch < 2; ++ch)
-        if (__any_sync(0xffffffffu, any_a[ch]) && lane == 0) atomicOr(const_cast<int32_t*>(&info[1 + rh * 2 + ch]), 1);
-    } else {
-      if (__any_sync(0xffffffffu, any_a[0] || any_a[1]) && lane == 0) atomicOr(const_cast<int32_t*>(&info[1]), 1);
-    }
-    tc_fence_before();
-    __syncthreads();
-    if (tid == 0) {
+    // tile "any" flags: a warp that saw a probability >= alpha writes the flag itself (every writer stores 1)
+    {
       int32_t* tf = p.tile_flag + (int64_t)h * p.n_la_bits;
       if (T == 64) {
-        for (int a = 0; a < 2; ++a)
-          for (int b = 0; b < 2; ++b) {
-            const int ti = 2 * i + a, tj = 2 * j + b;
-            if (info[1 + a * 2 + b] && tj <= ti && ti < pt) tf[ti * (ti + 1) / 2 + tj] = 1;
-            info[1 + a * 2 + b] = 0;
-          }
+#pragma unroll
+        for (int ch = 0; ch < 2; ++ch) {
+          const int ti = 2 * i + rh, tj = 2 * j + ch;
+          if (__any_sync(0xffffffffu, any_a[ch]) && lane == 0 && tj <= ti && ti < pt) tf[ti * (ti + 1) / 2 + tj] = 1;
+        }
       } else {
-        if (info[1]) tf[i * (i + 1) / 2 + j] = 1;
-        info[1] = 0;
+        if (__any_sync(0xffffffffu, any_a[0] || any_a[1]) && lane == 0) tf[i * (i + 1) / 2 + j] = 1;
       }
     }
-    __syncthreads();
+    tc_fence_before();
+    __syncthreads();            // every warp has read S[st]: the MMA of block j + 2 may overwrite it
   }
   tc_fence_before();
   __syncthreads();
