@@ -100,10 +100,12 @@ struct Smem {
   static constexpr int bVFull = bKEmpty + kKStages, bVEmpty = bVFull + kVStages;
   static constexpr int bSFull = bVEmpty + kVStages, bPFull = bSFull + kNQ, bODone = bPFull + kNQ * kPvParts;   // bPFull + part * kNQ + q
   static constexpr int bItemFull = bODone + kNQ, bItemEmpty = bItemFull + 2;
-  static constexpr int kNumBars = bItemEmpty + 2;
+  static constexpr int bInfoFull = bItemEmpty + 2;      // the item warp has decoded the item of this slot (for the softmax warpgroups)
+  static constexpr int kNumBars = bInfoFull + 2;
   static constexpr int kInfoOff = kBarOff + ((kNumBars * 8 + 15) / 16) * 16;
-  // info words: [0] tmem base, [1..2] item ring, [3] "the item has MMA steps" (item warp -> MMA issuer), [4 .. 4+kKStages) per-K-stage step info
-  static constexpr int kBytes = kInfoOff + 64;
+  // info words: [0] tmem base, [1..2] item ring, [3] "the item has MMA steps" (item warp -> MMA issuer), [4 .. 4+kKStages) per-K-stage step info,
+  // [16 .. 48) the decoded work items of the two ring slots (item warp -> softmax warpgroups, 16 words each)
+  static constexpr int kBytes = kInfoOff + 64 + 2 * 64;
   static_assert(kBytes <= 227 * 1024, "shared memory budget");
 };
 
@@ -118,6 +120,25 @@ struct Item {
   int kbase;               // DENSE: first key row (first row of the prompt; 0 with one prompt and in the comparator)
   int lptr[kNQ], lcnt[kNQ];  // DOC: local list of each tile
 };
+
+// what a softmax warpgroup needs of a work item, as the item warp publishes it through shared memory (16 words per ring
+// slot): the dependent global loads of load_item plus the diagonal test then run once, a whole item ahead, instead of at
+// the start of every item on the warpgroup's own path
+struct ItemInfo {
+  int h, is_dense, c0, cp, kbase, row0[kNQ], rows[kNQ], lcnt[kNQ], diag[kNQ];
+};
+__device__ __forceinline__ void publish_item(volatile int32_t* w, const Item& it, const int (&diag)[kNQ]) {
+  w[0] = it.h; w[1] = it.is_dense; w[2] = it.c0; w[3] = it.cp; w[4] = it.kbase;
+#pragma unroll
+  for (int q = 0; q < kNQ; ++q) { w[5 + q] = it.row0[q]; w[7 + q] = it.rows[q]; w[9 + q] = it.lcnt[q]; w[11 + q] = diag[q]; }
+}
+__device__ __forceinline__ ItemInfo read_item(const volatile int32_t* w) {
+  ItemInfo it;
+  it.h = w[0]; it.is_dense = w[1]; it.c0 = w[2]; it.cp = w[3]; it.kbase = w[4];
+#pragma unroll
+  for (int q = 0; q < kNQ; ++q) { it.row0[q] = w[5 + q]; it.rows[q] = w[7 + q]; it.lcnt[q] = w[9 + q]; it.diag[q] = w[11 + q]; }
+  return it;
+}
 
 __device__ __forceinline__ Item load_item(const AttnParams& p, int code) {
   Item it;
@@ -251,7 +272,9 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
       for (int part = 0; part < kPvParts; ++part) mbar_init(bar(S::bPFull + part * kNQ + q), 128);   // P of one key range written
       mbar_init(bar(S::bODone + q), 1);
     }
-    for (int i = 0; i < 2; ++i) { mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 7 + 128 * kNQ); }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(bar(S::bItemFull + i), 1); mbar_init(bar(S::bItemEmpty + i), 7 + 128 * kNQ); mbar_init(bar(S::bInfoFull + i), 1);
+    }
     fence_barrier_init();
     prefetch_tensormap(&tm_q); prefetch_tensormap(&tm_k); prefetch_tensormap(&tm_v);
     prefetch_tensormap(&tm_kg); prefetch_tensormap(&tm_vg);
@@ -302,6 +325,17 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
       code = __shfl_sync(0xffffffffu, code, 0);
       if (code < 0) break;
       const Item it = load_item(p, code);
+      {
+        int diag[kNQ];
+#pragma unroll
+        for (int q = 0; q < kNQ; ++q)
+          diag[q] = !it.is_dense && it.lcnt[q] > 0 &&
+                    p.local_idx[(int64_t)it.h * p.local_cap + it.lptr[q] + it.lcnt[q] - 1] == it.tile_id[q];
+        if (lane == 0) {
+          publish_item(info + 16 + 16 * slot, it, diag);
+          mbar_arrive(bar(S::bInfoFull + slot));
+        }
+      }
       // ---- Q tiles
       mbar_wait(bar(S::bQEmpty), (it_n & 1) ^ 1, 101);
       if (lane == 0) {
@@ -532,22 +566,22 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
       const int slot = it_n & 1;
       mbar_wait(bar(S::bItemFull + slot), (it_n >> 1) & 1, 300);
       const int code = info[1 + slot];
-      mbar_arrive(bar(S::bItemEmpty + slot));
-      if (code < 0) break;
+      if (code < 0) { mbar_arrive(bar(S::bItemEmpty + slot)); break; }
       int row0, rows, h, ngroups, nsteps, diag_step, lim, c0;
       bool paged_item;
       {
-        const Item it = load_item(p, code);
+        mbar_wait(bar(S::bInfoFull + slot), (it_n >> 1) & 1, 304);
+        const ItemInfo it = read_item(info + 16 + 16 * slot);
+        mbar_arrive(bar(S::bItemEmpty + slot));
         row0 = q ? it.row0[1] : it.row0[0]; rows = q ? it.rows[1] : it.rows[0]; h = it.h;
-        const int lcnt = q ? it.lcnt[1] : it.lcnt[0], lptr = q ? it.lptr[1] : it.lptr[0];
-        const int tile_id = q ? it.tile_id[1] : it.tile_id[0];
+        const int lcnt = q ? it.lcnt[1] : it.lcnt[0];
+        const int diag = q ? it.diag[1] : it.diag[0];
         if (rows <= 0) continue;
         c0 = it.c0;
         ngroups = it.is_dense ? 0 : (p.paged ? it.cp - it.c0 : (it.cp - it.c0 + kBN - 1) / kBN);
         nsteps = it.is_dense ? dense_steps(row0 - it.kbase, rows) : ngroups + lcnt;
         diag_step = -1;                                   // the step (if any) that is the causally masked diagonal tile
-        if (!it.is_dense && lcnt > 0 && p.local_idx[(int64_t)h * p.local_cap + lptr + lcnt - 1] == tile_id)
-          diag_step = nsteps - 1;
+        if (diag) diag_step = nsteps - 1;
         // columns [0, lim) of the current step are allowed for this row; lim drops by kBN per step in the cross
         // phase (ragged last group) and in DENSE items (causal frontier)
         lim = it.is_dense ? row0 - it.kbase + r + 1 : it.cp - it.c0;
