@@ -1,6 +1,7 @@
 /* Plain-C client of include/sift.h (no Python, no torch): proves the boundary is a C ABI.
  *   abi_smoke host   -> host-only calls: version, layout arithmetic, error codes        (runs without a GPU)
- *   abi_smoke gpu    -> decode + dense/sparse attention on a small prompt through cudaMalloc'd buffers
+ *   abi_smoke gpu    -> decode + dense/sparse attention on a small prompt through cudaMalloc'd buffers, the same layer
+ *                       from host buffers, two prompts in one call, the paper's index layout
  * Expected values are closed forms: all-ones bit vectors => counts are sizes; Q = 0 => uniform attention, so every
  * output row is the running mean of the V rows it may see, and LSE = ln(#keys). */
 #include <math.h>
@@ -133,6 +134,47 @@ static int gpu_part(void) {
     CHECK(sift_host_ctx_destroy(ctx) == SIFT_OK);
     cudaStreamDestroy(st); cudaFree(d_ws);
     cudaFreeHost(p_la); cudaFreeHost(p_ca); cudaFreeHost(p_q); cudaFreeHost(p_k); cudaFreeHost(p_v); cudaFreeHost(p_o); cudaFreeHost(p_lse);
+  }
+  /* two prompts in one call (sift_shape.n_prompts): the same prompt twice, packed back to back; every row must see its own
+   * prompt only, i.e. both halves of O and LSE repeat the single-prompt result bit for bit.  Then the paper's index layout. */
+  {
+    int32_t off2[5] = {0, L0, L0 + L1, 2 * L0 + L1, 2 * (L0 + L1)}, pstart[3] = {0, 2, 4}, pq[2] = {LQ, LQ};
+    sift_shape s2 = {sizeof(sift_shape), 1, HQ, HKV, D, 4, 0, T, 1, off2, 2, pstart, pq};
+    sift_md_layout lay2;
+    CHECK(sift_metadata_layout(&s2, &lay2) == SIFT_OK && lay2.n_tokens == 2 * N && lay2.n_seg == 6 && lay2.n_tiles == 2 * lay.n_tiles);
+    int64_t la_off2[4] = {la_off[0], la_off[1], la_off[0], la_off[1]}, ca_off2[4] = {ca_off[0], ca_off[1], ca_off[0], ca_off[1]};
+    void *d_md2, *d_q2, *d_k2, *d_v2, *d_o2, *d_lse2, *d_ptr, *d_idx;
+    CHECK(cudaMalloc(&d_md2, lay2.total_bytes) == 0 && cudaMalloc(&d_q2, 2 * qb) == 0 && cudaMalloc(&d_k2, 2 * kb) == 0 &&
+          cudaMalloc(&d_v2, 2 * kb) == 0 && cudaMalloc(&d_o2, 2 * qb) == 0 && cudaMalloc(&d_lse2, (size_t)HQ * 2 * N * 4) == 0);
+    for (int rep = 0; rep < 2; ++rep)
+      CHECK(cudaMemcpy((char*)d_q2 + rep * qb, hq, qb, 1) == 0 && cudaMemcpy((char*)d_k2 + rep * kb, hk, kb, 1) == 0 &&
+            cudaMemcpy((char*)d_v2 + rep * kb, hv, kb, 1) == 0);
+    CHECK(sift_decode_metadata(&s2, (const uint8_t*)d_la, la_off2, (const uint8_t*)d_ca, ca_off2, d_md2, lay2.total_bytes, NULL) == SIFT_OK);
+    CHECK(sift_prefill_attention(&s2, 0, d_q2, d_k2, d_v2, HQ * D, HKV * D, HKV * D, d_md2, d_o2, HQ * D, (float*)d_lse2, 0.f, NULL) == SIFT_OK);
+    uint16_t* ho2 = (uint16_t*)malloc(2 * qb);
+    float* hl2 = (float*)malloc((size_t)HQ * 2 * N * 4);
+    CHECK(cudaDeviceSynchronize() == 0 && cudaMemcpy(ho2, d_o2, 2 * qb, 2) == 0 && cudaMemcpy(hl2, d_lse2, (size_t)HQ * 2 * N * 4, 2) == 0);
+    for (int rep = 0; rep < 2; ++rep) {
+      CHECK(memcmp((char*)ho2 + rep * qb, ho_sparse, qb) == 0);
+      for (int h = 0; h < HQ; ++h) CHECK(memcmp(hl2 + (size_t)h * 2 * N + rep * N, hl_sparse + (size_t)h * N, (size_t)N * 4) == 0);
+    }
+    /* sparse_n_indices as the paper lays it out from the single-prompt metadata: all bits are set,
+     * so the list of document tile (d, i) is [all keys of the earlier documents] ++ [tiles 0..i of d] */
+    int64_t hp[HQ * 16];
+    CHECK(lay.n_tiles + 1 <= 16 && cudaMalloc(&d_ptr, sizeof(hp)) == 0);
+    CHECK(sift_paper_index_offsets(&s, 0, d_md, (int64_t*)d_ptr, NULL) == SIFT_OK);
+    CHECK(cudaDeviceSynchronize() == 0 && cudaMemcpy(hp, d_ptr, (size_t)HQ * (lay.n_tiles + 1) * 8, 2) == 0);
+    /* doc 0: 4 tiles with 1,2,3,4 entries; doc 1: 3 tiles with L0 + 1,2,3; query tile (id 7): 8 */
+    const int64_t want_total = 10 + 3 * (int64_t)L0 + 6 + 8;
+    for (int h = 0; h < HQ; ++h) CHECK(hp[h * (lay.n_tiles + 1) + 0] == 0 && hp[h * (lay.n_tiles + 1) + 4] == 10 && hp[h * (lay.n_tiles + 1) + lay.n_tiles] == want_total);
+    CHECK(cudaMalloc(&d_idx, (size_t)HQ * want_total * 4) == 0);
+    CHECK(sift_export_paper_indices(&s, 0, d_md, (const int64_t*)d_ptr, (int32_t*)d_idx, want_total, NULL) == SIFT_OK);
+    int32_t* hidx = (int32_t*)malloc((size_t)HQ * want_total * 4);
+    CHECK(cudaDeviceSynchronize() == 0 && cudaMemcpy(hidx, d_idx, (size_t)HQ * want_total * 4, 2) == 0);
+    for (int i = 0; i < L0; ++i) CHECK(hidx[10 + i] == i);              /* first tile of doc 1: the L0 keys of doc 0 ... */
+    CHECK(hidx[10 + L0] == 4);                                          /* ... then its own tile (global id 4) */
+    free(ho2); free(hl2); free(hidx);
+    cudaFree(d_md2); cudaFree(d_q2); cudaFree(d_k2); cudaFree(d_v2); cudaFree(d_o2); cudaFree(d_lse2); cudaFree(d_ptr); cudaFree(d_idx);
   }
   cudaFree(d_la); cudaFree(d_ca); cudaFree(d_md); cudaFree(d_q); cudaFree(d_k); cudaFree(d_v); cudaFree(d_o); cudaFree(d_lse);
   printf("abi_smoke gpu ok\n");
