@@ -10,9 +10,10 @@ from . import api
 
 
 class HostLayerPipeline:
-    def __init__(self, prompt_shape, device: str = "cuda"):
+    def __init__(self, prompt_shape, device: str = "cuda", shape: "api.Shape" = None):
+        """prompt_shape: workload.PromptShape of one prompt; or shape: an api.Shape (e.g. Shape.from_batch)."""
         self.ps = prompt_shape
-        self.shape = api.Shape.from_prompt(prompt_shape)
+        self.shape = shape if shape is not None else api.Shape.from_prompt(prompt_shape)
         self.device = torch.device(device)
         self.ctx = api.HostContext()
         self.ws = None

@@ -118,3 +118,22 @@ def test_batch_of_c2_prompts_runs_and_matches_single_calls():
         o1, lse1 = api.sift_prefill_attention(s1, 0, q[lo:hi].contiguous(), k[lo:hi].contiguous(), v[lo:hi].contiguous(), md1)
         torch.cuda.synchronize()
         assert torch.equal(o[lo:hi], o1) and torch.equal(lse[:, lo:hi], lse1)
+
+
+def test_host_pipeline_on_a_batch_matches_the_device_call():
+    """sift_prefill_layer_host with several prompts: per kv-head group from HOST buffers, bit-identical to the device call."""
+    from paper_2606_09441_b200.pipeline import HostLayerPipeline
+    b = _batch(1, 128, 128, (4, 2))
+    shape, md = _decode(b)
+    layer = 1
+    q, k, v = b.qkv(layer)
+    o_ref, lse_ref = api.sift_prefill_attention(shape, layer, q.cuda(), k.cuda(), v.cuda(), md)
+    torch.cuda.synchronize()
+    qh, kh, vh = (t.pin_memory() for t in (q, k, v))
+    la_h, ca_h = torch.from_numpy(b.la_blob).pin_memory(), torch.from_numpy(b.ca_blob).pin_memory()
+    o_h = torch.empty(q.shape, dtype=q.dtype).pin_memory()
+    lse_h = torch.empty(lse_ref.shape, dtype=torch.float32).pin_memory()
+    pipe = HostLayerPipeline(None, shape=shape)
+    pipe.run(la_h, ca_h, b.la_doc_off, b.ca_doc_off, qh, kh, vh, o_h, layer=layer, lse_h=lse_h)
+    pipe.wait()
+    assert torch.equal(o_h, o_ref.cpu()) and torch.equal(lse_h, lse_ref.cpu())
