@@ -74,3 +74,30 @@ def test_fp8_rejects_head_dim_64():
     k8 = torch.zeros((w.shape.n_tokens, 1, 64), dtype=torch.uint8, device="cuda")
     with pytest.raises(api.SiftError):
         api.sift_prefill_attention_fp8(shape, 0, q8, k8, k8, [1, 1], [1], [1], md)
+
+
+def test_fp8_on_a_batch_of_prompts():
+    """e4m3 Q/K/V and several prompts in one call go through the same kernel body: sampled rows against the oracle (Part 5
+    on the values Part 6 decodes)."""
+    kw = dict(n_layers=1, n_q_heads=4, n_kv_heads=2, head_dim=128, tile=128, cross_gran=1)
+    b = wl.make_batch("f8b", [wl.custom("a", doc_lens=(300, 260), query_len=50, p_loc=0.5, p_cross=0.4, seed=71, **kw),
+                              wl.custom("b", doc_lens=(129, 500, 64), query_len=130, p_loc=0.5, p_cross=0.3, seed=72, **kw)])
+    sh = b.head_shape
+    shape = api.Shape.from_batch(b)
+    la, ca = torch.from_numpy(b.la_blob).cuda(), torch.from_numpy(b.ca_blob).cuda()
+    md = api.sift_decode_metadata(shape, la, b.la_doc_off, ca, b.ca_doc_off)
+    q, k, v = b.qkv(0)
+    (q8, qs), (k8, ks), (v8, vs) = wl.quantize_e4m3(q), wl.quantize_e4m3(k), wl.quantize_e4m3(v)
+    o, lse = api.sift_prefill_attention_fp8(shape, 0, q8.cuda(), k8.cuda(), v8.cuda(), qs, ks, vs, md)
+    torch.cuda.synchronize()
+    o, lse = o.float().cpu(), lse.cpu()
+    deq = lambda x8, s: torch.from_numpy(so.e4m3_decode(x8.numpy()) * s.astype(np.float64)[None, :, None]).float()
+    qd, kd, vd = deq(q8, qs), deq(k8, ks), deq(v8, vs)
+    rows = list(range(0, b.n_tokens, 7)) + [b.n_tokens - 1]
+    n_docs = len(b.doc_lens)
+    for h in range(sh.n_q_heads):
+        lav = [b.la_vec(0, h, d) for d in range(n_docs)]
+        cav = [b.ca_vec(0, h, d) for d in range(n_docs)]
+        ro, rl = so.sift_attention_rows_batch(qd, kd, vd, h, b.prompts, sh.tile, 1, lav, cav, rows)
+        d = (o[rows, h] - ro).abs()
+        assert float(d.max()) <= TOL8_MAX and float(d.mean()) <= TOL8_MEAN and float((lse[h, rows] - rl).abs().max()) <= gu.TOL_LSE
