@@ -198,6 +198,39 @@ int sift_encode_document(int32_t doc_len, int32_t n_q_heads, int32_t n_kv_heads,
                          const float* lse, float alpha, float beta, float gamma, float softmax_scale,
                          uint8_t* la_out, uint8_t* ca_out, void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- sift_encode_document for callers that cannot allocate device memory ----
+ * sift_encode_document needs a scratch workspace, and a caller has to get that from somewhere.  Some cannot: a plug-in
+ * or custom op that is handed its input and output buffers by a host framework and has no handle on that framework's
+ * allocator; a serving process that gave all free HBM to its KV-cache pool at start-up, where a cudaMalloc may fail
+ * and, if it succeeds, stalls every stream of the device while it runs.  sift_encode_document_static is the same
+ * operation (same arguments minus the workspace, same kernels, bit-identical la_out / ca_out) with the scratch in a
+ * fixed array that is part of the library's device image: SIFT_ENCODE_STATIC_SCRATCH_BYTES on every GPU the library
+ * is used on, held from the moment the CUDA runtime loads the library's kernels on that GPU until the process exits.
+ * The call itself makes no cudaMalloc / cudaFree and uses no routine that allocates.
+ *   Limit     sift_encode_workspace_size(doc_len, n_q_heads, tile) <= SIFT_ENCODE_STATIC_SCRATCH_BYTES (4 MiB), i.e.
+ *             n_q_heads * (doc_len rounded up to 128 + P(P+1)/2) * 4 bytes with P = ceil(doc_len / tile): 32 q-heads of a
+ *             12,288-token document at tile 64, of a 16,384-token one at tile 128 (the paper's documents are <= 4096
+ *             tokens).  Anything larger returns SIFT_ERR_WORKSPACE with the two sizes in sift_last_error() and enqueues
+ *             nothing; encode fewer heads per call (Q, lse, la_out, ca_out are per-head slices) or use the workspace
+ *             variant.
+ *   Set-up    the first call on each device looks up the array's address on that device (cudaGetSymbolAddress, which
+ *             may also make the runtime load the library's device code there) and keeps it; make that first call with
+ *             the device current as for every other call, and make it before any stream capture is begun.  Later calls
+ *             on that device do no set-up.  Thread-safe.
+ *   Sharing   there is ONE array per GPU and every call on that GPU uses it.  A call first clears the part it needs,
+ *             on `stream` (what the previous call left there is never read), so calls issued to one stream, or otherwise
+ *             ordered one after the other, are independent.  Two calls that may run on the GPU at the same time (different
+ *             streams without an event between them, two host threads, two libraries' worth of users in one process)
+ *             race on the array and produce wrong bits without any error: order them, or give all but one of them a
+ *             workspace through sift_encode_document.
+ * Everything else (arguments, outputs, errors, stream semantics) is as in sift_encode_document. */
+#define SIFT_ENCODE_STATIC_SCRATCH_BYTES (4u << 20)
+size_t sift_encode_static_scratch_bytes(void); /* the value the library was built with */
+int sift_encode_document_static(int32_t doc_len, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim, int32_t tile,
+                                int32_t cross_gran, const void* Q, const void* K, int64_t q_row_stride, int64_t k_row_stride,
+                                const float* lse, float alpha, float beta, float gamma, float softmax_scale,
+                                uint8_t* la_out, uint8_t* ca_out, void* stream);
+
 /* ---- the paper's own index layout (sec 5.1) ----
  * sparse_n_indices as the paper stores it: per (head, M-block t) ONE packed int32 list, the CA entries of all earlier
  * documents of the prompt first (key rows at G = 1, global tile ids at G = tile), then the M-block's LA entries (global

@@ -18,7 +18,7 @@ EXPORTS = ("sift_version", "sift_last_error", "sift_metadata_size", "sift_metada
            "sift_encode_workspace_size", "sift_encode_output_sizes", "sift_encode_document",
            "sift_host_ctx_create", "sift_host_ctx_destroy", "sift_prefill_layer_host_workspace_size",
            "sift_prefill_layer_host", "sift_paper_index_offsets", "sift_export_paper_indices",
-           "sift_prefill_attention_fp8")
+           "sift_prefill_attention_fp8", "sift_encode_document_static", "sift_encode_static_scratch_bytes")
 
 
 class SiftShape(C.Structure):
@@ -71,6 +71,8 @@ def lib() -> C.CDLL:
                                            C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_float, C.c_float, C.c_float,
                                            C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.sift_encode_output_sizes.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+        L.sift_encode_static_scratch_bytes.restype = C.c_size_t
+        L.sift_encode_document_static.argtypes = L.sift_encode_document.argtypes[:-3] + [C.c_void_p]
         L.sift_host_ctx_create.argtypes = [C.POINTER(C.c_void_p)]
         L.sift_host_ctx_destroy.argtypes = [C.c_void_p]
         L.sift_prefill_layer_host_workspace_size.argtypes = [C.POINTER(SiftShape), C.c_size_t, C.c_size_t, C.POINTER(C.c_size_t)]
@@ -273,6 +275,37 @@ def sift_encode_document(q: torch.Tensor, k: torch.Tensor, lse: torch.Tensor, ti
                                       lse.data_ptr(), alpha, beta, gamma, softmax_scale, la.data_ptr(), ca.data_ptr(),
                                       ws.data_ptr(), nb.value, _stream(stream)), "sift_encode_document")
     return la, ca
+
+
+def sift_encode_static_scratch_bytes() -> int:
+    """Size of the encoder's built-in scratch array (include/sift.h: SIFT_ENCODE_STATIC_SCRATCH_BYTES)."""
+    return int(lib().sift_encode_static_scratch_bytes())
+
+
+def sift_encode_document_static(q: torch.Tensor, k: torch.Tensor, lse: torch.Tensor, la: torch.Tensor, ca: torch.Tensor,
+                                tile: int, cross_gran: int = 1, alpha: float = 1e-3, beta: float = 1e-2,
+                                gamma: float = 0.1, softmax_scale: float = 0.0, stream=None) -> None:
+    """sift_encode_document for a caller that may not allocate device memory (include/sift.h): the scratch is an array
+    inside the library, so this wrapper allocates nothing either and the caller hands in the outputs, la [Hq, la_bytes]
+    and ca [Hq, ca_bytes] uint8 CUDA (sizes from sift_encode_output_sizes).  Documents whose scratch exceeds
+    sift_encode_static_scratch_bytes() raise SiftError.  All calls on one GPU share that one array: keep them ordered."""
+    assert q.is_cuda and k.is_cuda and lse.is_cuda and q.dtype == torch.bfloat16 and k.dtype == torch.bfloat16
+    assert lse.dtype == torch.float32 and lse.is_contiguous() and q.stride(2) == 1 and k.stride(2) == 1
+    assert q.stride(1) == q.shape[2] and k.stride(1) == k.shape[2]
+    n, hq, d = q.shape
+    la_bytes, ca_bytes = sift_encode_output_sizes(n, tile, cross_gran)
+    for t, nb in ((la, la_bytes), (ca, ca_bytes)):
+        assert t.is_cuda and t.dtype == torch.uint8 and t.is_contiguous() and tuple(t.shape) == (hq, nb), (t.shape, (hq, nb))
+    _check(lib().sift_encode_document_static(n, hq, k.shape[1], d, tile, cross_gran, q.data_ptr(), k.data_ptr(), q.stride(0),
+                                             k.stride(0), lse.data_ptr(), alpha, beta, gamma, softmax_scale, la.data_ptr(),
+                                             ca.data_ptr(), _stream(stream)), "sift_encode_document_static")
+
+
+def sift_encode_output_sizes(doc_len: int, tile: int, cross_gran: int) -> Tuple[int, int]:
+    """Bytes of one q-head's LA / CA vector of a document (include/sift.h)."""
+    lb, cb = C.c_size_t(), C.c_size_t()
+    _check(lib().sift_encode_output_sizes(doc_len, tile, cross_gran, C.byref(lb), C.byref(cb)), "sift_encode_output_sizes")
+    return int(lb.value), int(cb.value)
 
 
 class HostContext:

@@ -12,6 +12,7 @@
 #include <cuda_bf16.h>
 #include <math.h>
 #include <string.h>
+#include <mutex>
 
 #include "sift_common.h"
 #include "sm100_ptx.cuh"
@@ -297,4 +298,63 @@ extern "C" int sift_encode_document(int32_t doc_len, int32_t n_q_heads, int32_t 
   if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "encode launch: %s", cudaGetErrorString(e));
   count_launch(2);
   return SIFT_OK;
+}
+
+// ---- sift_encode_document_static: the encoder for callers that have no device allocator (include/sift.h) ----
+// The per-key counters and per-tile flags that sift_encode_document keeps in a caller-supplied workspace live here in
+// a fixed array inside the library's device image.  The CUDA runtime places it in every GPU's memory when the module is
+// loaded there and releases it when the process exits: SIFT_ENCODE_STATIC_SCRATCH_BYTES per GPU, used or not.
+static __device__ __align__(256) unsigned char g_encode_static_scratch[SIFT_ENCODE_STATIC_SCRATCH_BYTES];
+
+namespace sift {
+// In host code `g_encode_static_scratch` is only the host-side handle of the symbol, not a device address; the address
+// a kernel can use differs per GPU and is looked up once per device, with that device current, and remembered here.
+constexpr int kMaxStaticDevices = 64;
+static std::mutex g_static_mu;
+static void* g_static_ptr[kMaxStaticDevices];   // device address of the array on device i, NULL until its first call
+
+static int encode_static_scratch(void** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return set_error(SIFT_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+  if (dev < 0 || dev >= kMaxStaticDevices) return set_error(SIFT_ERR_UNSUPPORTED, "device ordinal %d >= %d", dev, kMaxStaticDevices);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    void* ptr = nullptr;
+    e = cudaGetSymbolAddress(&ptr, g_encode_static_scratch);
+    if (e != cudaSuccess || !ptr) {
+      cudaGetLastError();
+      return set_error(SIFT_ERR_CUDA, "cudaGetSymbolAddress(static encoder scratch) on device %d: %s", dev, cudaGetErrorString(e));
+    }
+    g_static_ptr[dev] = ptr;
+  }
+  *out = g_static_ptr[dev];
+  return SIFT_OK;
+}
+}  // namespace sift
+
+extern "C" size_t sift_encode_static_scratch_bytes(void) { return (size_t)SIFT_ENCODE_STATIC_SCRATCH_BYTES; }
+
+extern "C" int sift_encode_document_static(int32_t doc_len, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
+                                           int32_t tile, int32_t cross_gran, const void* Q, const void* K,
+                                           int64_t q_row_stride, int64_t k_row_stride, const float* lse, float alpha,
+                                           float beta, float gamma, float softmax_scale, uint8_t* la_out, uint8_t* ca_out,
+                                           void* stream) {
+  int rc = enc_check(doc_len, n_q_heads, n_kv_heads, head_dim, tile, cross_gran);
+  if (rc) return rc;
+  size_t need = 0;
+  if ((rc = sift_encode_workspace_size(doc_len, n_q_heads, tile, &need))) return rc;
+  if (need > (size_t)SIFT_ENCODE_STATIC_SCRATCH_BYTES)
+    return set_error(SIFT_ERR_WORKSPACE,
+                     "sift_encode_document_static: doc_len %d x %d q-heads at tile %d needs %zu bytes of scratch, the "
+                     "built-in array holds %zu (SIFT_ENCODE_STATIC_SCRATCH_BYTES); use sift_encode_document with a "
+                     "workspace of your own, or encode fewer heads per call",
+                     doc_len, n_q_heads, tile, need, (size_t)SIFT_ENCODE_STATIC_SCRATCH_BYTES);
+  void* scratch = nullptr;
+  if ((rc = encode_static_scratch(&scratch))) return rc;
+  // From here on it is the ordinary encoder on the built-in scratch: it clears the `need` bytes it uses on `stream`
+  // (the array still holds the previous call's counts), runs the score and pack kernels, and allocates nothing.
+  return sift_encode_document(doc_len, n_q_heads, n_kv_heads, head_dim, tile, cross_gran, Q, K, q_row_stride, k_row_stride,
+                              lse, alpha, beta, gamma, softmax_scale, la_out, ca_out, scratch,
+                              (size_t)SIFT_ENCODE_STATIC_SCRATCH_BYTES, stream);
 }
