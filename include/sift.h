@@ -97,11 +97,18 @@ typedef struct {
   int32_t n_tokens;  /* N */
   size_t seg_info;   /* private: per segment {document index or -1, first document of its prompt, first row of its prompt, first tile of its prompt} */
 } sift_md_layout;
+/* The struct before n_seg / n_tokens / seg_info were added.  A caller that passes a shape of SIFT_SHAPE_SIZE_V1 bytes
+ * was built against that older header and owns a sift_md_layout of this size: sift_metadata_layout then writes
+ * exactly SIFT_MD_LAYOUT_SIZE_V1 bytes (struct_size says so) and nothing behind them.  The offsets and total_bytes
+ * are the same either way; total_bytes already covers the private arrays. */
+#define SIFT_MD_LAYOUT_SIZE_V1 ((uint32_t)offsetof(sift_md_layout, n_seg))
 
 const char* sift_version(void);
 const char* sift_last_error(void);
 
-/* Size / layout of the metadata buffer for a shape.  Pure host arithmetic. */
+/* Size / layout of the metadata buffer for a shape.  Pure host arithmetic.  sift_metadata_layout writes
+ * sizeof(sift_md_layout) bytes to `out`, or SIFT_MD_LAYOUT_SIZE_V1 bytes when shape->struct_size is SIFT_SHAPE_SIZE_V1
+ * (see above); out->struct_size holds the number of bytes written. */
 int sift_metadata_size(const sift_shape* shape, size_t* bytes);
 int sift_metadata_layout(const sift_shape* shape, sift_md_layout* out);
 

@@ -124,6 +124,10 @@ class Shape:
         self.doc_offsets = np.ascontiguousarray(self.doc_offsets, dtype=np.int32)
         ip = C.POINTER(C.c_int32)
         n_prompts, pds, pql = 0, ip(), ip()
+        if self.prompt_query_len is not None and len(self.prompt_query_len) == 1:
+            # the library reads n_prompts <= 1 as "one prompt" and takes query_len: say it that way here too
+            self.query_len = int(np.asarray(self.prompt_query_len)[0])
+            self.prompt_doc_start = self.prompt_query_len = None
         if self.prompt_doc_start is not None:
             self.prompt_doc_start = np.ascontiguousarray(self.prompt_doc_start, dtype=np.int32)
             self.prompt_query_len = np.ascontiguousarray(self.prompt_query_len, dtype=np.int32)
@@ -150,10 +154,8 @@ class Shape:
 
     @property
     def n_tokens(self) -> int:
-        if self.prompt_query_len is not None and len(self.prompt_query_len) > 1:
+        if self.prompt_query_len is not None:   # two or more prompts (__post_init__ folds one prompt into query_len)
             return int(self.doc_offsets[-1]) + int(self.prompt_query_len.sum())
-        if self.prompt_query_len is not None and len(self.prompt_query_len) == 1:
-            return int(self.doc_offsets[-1]) + int(self.prompt_query_len[0])
         return int(self.doc_offsets[-1]) + self.query_len
 
     @property

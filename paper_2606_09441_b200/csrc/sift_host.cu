@@ -228,7 +228,14 @@ int64_t sift_launch_count(void) { return g_launches.load(std::memory_order_relax
 
 int sift_metadata_layout(const sift_shape* shape, sift_md_layout* out) {
   if (!out) return set_error(SIFT_ERR_INVALID_ARG, "out is NULL");
-  return compute_layout(shape, out);
+  sift_md_layout lay;
+  int rc = compute_layout(shape, &lay);
+  if (rc) return rc;
+  // a V1-sized shape comes from a caller whose sift_md_layout ends before n_seg: write no more than it owns
+  const size_t n = shape->struct_size == SIFT_SHAPE_SIZE_V1 ? (size_t)SIFT_MD_LAYOUT_SIZE_V1 : sizeof(lay);
+  lay.struct_size = (uint32_t)n;
+  memcpy(out, &lay, n);
+  return SIFT_OK;
 }
 
 int sift_metadata_size(const sift_shape* shape, size_t* bytes) {

@@ -26,6 +26,14 @@ struct HostCtx {
 
 static size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 
+// A caller built against the older header passes a shape of SIFT_SHAPE_SIZE_V1 bytes: read no further than it says
+// (validate_shape has accepted struct_size), the prompt fields it does not have read as "one prompt".
+static void copy_shape(const sift_shape* s, sift_shape* out) {
+  memset(out, 0, sizeof(*out));
+  memcpy(out, s, s->struct_size < sizeof(*out) ? s->struct_size : sizeof(*out));
+  out->struct_size = sizeof(*out);
+}
+
 // Device workspace: Q | K | V | O | LSE | LA blob | CA blob | one metadata buffer per kv-head group
 struct HostLayout {
   size_t q, k, v, o, lse, la, ca, md, md_stride, total;
@@ -37,7 +45,8 @@ static int host_layout(const sift_shape* s, size_t la_bytes, size_t ca_bytes, Ho
   if (rc) return rc;
   const int64_t n = shape_n_tokens(s);
   const int hpg = s->n_q_heads / s->n_kv_heads;
-  sift_shape sub = *s;
+  sift_shape sub;
+  copy_shape(s, &sub);
   sub.n_layers = 1; sub.n_q_heads = hpg; sub.n_kv_heads = 1;
   if ((rc = compute_layout(&sub, &out->sub_lay))) return rc;
   size_t o = 0;
@@ -65,15 +74,27 @@ using namespace sift;
     if (e_ != cudaSuccess) return set_error(SIFT_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e_));  \
   } while (0)
 
-extern "C" int sift_host_ctx_create(sift_host_ctx** out) {
-  if (!out) return set_error(SIFT_ERR_INVALID_ARG, "out is NULL");
-  HostCtx* c = new HostCtx();
+extern "C" int sift_host_ctx_destroy(sift_host_ctx* ctx);
+
+static int ctx_init(HostCtx* c) {
   SIFT_CUDA_TRY(cudaGetDevice(&c->device), "cudaGetDevice");
   SIFT_CUDA_TRY(cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking), "cudaStreamCreate");
   SIFT_CUDA_TRY(cudaStreamCreateWithFlags(&c->s_cmp, cudaStreamNonBlocking), "cudaStreamCreate");
   SIFT_CUDA_TRY(cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking), "cudaStreamCreate");
   SIFT_CUDA_TRY(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming), "cudaEventCreate");
   SIFT_CUDA_TRY(cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming), "cudaEventCreate");
+  return SIFT_OK;
+}
+
+extern "C" int sift_host_ctx_create(sift_host_ctx** out) {
+  if (!out) return set_error(SIFT_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  HostCtx* c = new HostCtx();
+  const int rc = ctx_init(c);
+  if (rc) {   // whatever was created before the failure goes with the ctx
+    sift_host_ctx_destroy(reinterpret_cast<sift_host_ctx*>(c));
+    return rc;
+  }
   *out = reinterpret_cast<sift_host_ctx*>(c);
   return SIFT_OK;
 }
@@ -151,7 +172,10 @@ extern "C" int sift_prefill_layer_host(sift_host_ctx* ctx, const sift_shape* sha
   const size_t d2 = (size_t)HD * 2, qp = (size_t)Hq * d2, kp = (size_t)Hkv * d2;   // device row pitches (dense)
   cudaStream_t user = (cudaStream_t)stream;
 
-  // everything below is ordered after the caller's stream, and the caller's stream waits for all of it
+  // everything below is ordered after the caller's stream, and the caller's stream waits for all of it -- also when a
+  // step fails half way: what was enqueued before the failure still reads the host buffers and writes the workspace,
+  // so the caller's stream is made to wait for the three streams before the error is returned
+  auto enqueue = [&]() -> int {
   SIFT_CUDA_TRY(cudaEventRecord(c->ev_start, user), "cudaEventRecord");
   SIFT_CUDA_TRY(cudaStreamWaitEvent(c->s_in, c->ev_start, 0), "cudaStreamWaitEvent");
   SIFT_CUDA_TRY(cudaStreamWaitEvent(c->s_cmp, c->ev_start, 0), "cudaStreamWaitEvent");
@@ -162,7 +186,8 @@ extern "C" int sift_prefill_layer_host(sift_host_ctx* ctx, const sift_shape* sha
   // 256 B per row make poor DMA descriptors; Q and O are copied per group
   SIFT_CUDA_TRY(cudaMemcpy2DAsync(kd, kp, K_host, (size_t)k_row_stride * 2, kp, n, cudaMemcpyHostToDevice, c->s_in), "H2D K");
   SIFT_CUDA_TRY(cudaMemcpy2DAsync(vd, kp, V_host, (size_t)v_row_stride * 2, kp, n, cudaMemcpyHostToDevice, c->s_in), "H2D V");
-  sift_shape sub = *shape;
+  sift_shape sub;
+  copy_shape(shape, &sub);
   sub.n_layers = 1; sub.n_q_heads = hpg; sub.n_kv_heads = 1;
   for (int g = 0; g < Hkv; ++g) {
     const int h0 = g * hpg;
@@ -192,4 +217,16 @@ extern "C" int sift_prefill_layer_host(sift_host_ctx* ctx, const sift_shape* sha
   SIFT_CUDA_TRY(cudaEventRecord(c->ev_done, c->s_out), "cudaEventRecord");
   SIFT_CUDA_TRY(cudaStreamWaitEvent(user, c->ev_done, 0), "cudaStreamWaitEvent");
   return SIFT_OK;
+  };
+  rc = enqueue();
+  if (rc) {
+    // best effort, return codes ignored: the error being reported is the first one (g_err keeps its text)
+    cudaEventRecord(c->ev_in[0], c->s_in);
+    cudaStreamWaitEvent(c->s_out, c->ev_in[0], 0);
+    cudaEventRecord(c->ev_cmp[0], c->s_cmp);
+    cudaStreamWaitEvent(c->s_out, c->ev_cmp[0], 0);
+    cudaEventRecord(c->ev_done, c->s_out);
+    cudaStreamWaitEvent(user, c->ev_done, 0);
+  }
+  return rc;
 }
