@@ -308,7 +308,8 @@ def test_host_pipeline_matches_single_call():
 
 
 def test_no_out_of_bounds_writes_guard_bands():
-    """Outputs sit between guard bands (compute-sanitizer is not available on the GPU pool): metadata, O and LSE of a
+    """Outputs sit between guard bands (compute-sanitizer exits 86 on the GPU pool, "compute-sanitizer is closed on this
+    pool and stays closed": commands and reply in profiles/r3_sanitizer.md): metadata, O and LSE of a
     ragged prompt with non-tile-multiple lengths; the bands must come back untouched."""
     w = wl.custom("guard", n_q_heads=4, n_kv_heads=2, head_dim=128, doc_lens=(130, 257, 1, 640, 77), query_len=61,
                   tile=128, p_cross=0.5, seed=37)
