@@ -315,6 +315,7 @@ def run_ours(args):
         extra["64k"] = {"n_tokens": c4.w.shape.n_tokens, "attention_ms": a4, "effective_tflops": c4.flops / (a4 * 1e-3) / 1e12,
                         "dense_causal_ms": d4, "dense_tflops": c4.dense_flops / (d4 * 1e-3) / 1e12, "decode_us": k4 * 1e3,
                         "frac_of_peak": c4.flops / (a4 * 1e-3) / 1e12 / peaks["bf16"], "marked_density": c4.flops / c4.dense_flops}
+        extra["64k"]["chunked_prefill_4"] = chunked_leg(c4, 4, max(3, min(10, args.steps // 2)))
         del c4
     if args.config == "32k" and world == 1 and not args.no_extra_legs:
         torch.cuda.empty_cache()
@@ -337,7 +338,8 @@ def run_ours(args):
     if "64k" in extra:
         e = extra["64k"]
         others["64k"] = {"ms": e["attention_ms"], "tflops": e["effective_tflops"], "frac": e["frac_of_peak"],
-                         "dense_tflops": e["dense_tflops"], "decode_us": e["decode_us"]}
+                         "dense_tflops": e["dense_tflops"], "decode_us": e["decode_us"],
+                         "chunked_prefill_4": e["chunked_prefill_4"]}
     if "paged_32k" in extra:
         e = extra["paged_32k"]
         others["paged_32k"] = {"ms": e["paged_attention_ms"], "tflops": e["paged_effective_tflops"], "frac": e["paged_frac_of_peak"],
@@ -518,6 +520,24 @@ def density_sweep_leg(base_case, peaks, steps):
                     "dense_ms_same_regime": dense_ms})
         del c
     return out
+
+
+def chunked_leg(case, n_chunks, steps):
+    """SURVEY 8(f)-3 / PAPER.md:L67: the prompt in n_chunks equal row ranges through sift_prefill_attention_rows (same
+    metadata, K/V resident), against the single call timed in the same regime (back to back, no idle).  The difference
+    per chunk = launch + grid ramp + tail of a smaller problem + the passed-over schedule entries."""
+    n = case.w.shape.n_tokens
+    cuts = [n * i // n_chunks for i in range(n_chunks + 1)]
+
+    def chunks():
+        for a, b in zip(cuts[:-1], cuts[1:]):
+            case.api.sift_prefill_attention_rows(case.shape, case.layer, a, b, case.q, case.k, case.v, case.md, case.o, case.lse)
+    for _ in range(2):
+        chunks(); case.attention()
+    ms_c = float(np.mean(time_each(chunks, steps)))
+    ms_w = float(np.mean(time_each(case.attention, steps)))
+    return {"chunks": n_chunks, "rows_per_chunk": n // n_chunks, "all_chunks_ms": ms_c, "single_call_ms_same_regime": ms_w,
+            "overhead_us_per_chunk": (ms_c - ms_w) * 1e3 / n_chunks, "ratio": ms_c / ms_w}
 
 
 def paged_leg(base_case, peaks, steps):

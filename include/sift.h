@@ -132,6 +132,26 @@ int sift_prefill_attention(const sift_shape* shape, int32_t layer,
                            const void* metadata /*dev, from sift_decode_metadata*/,
                            void* O, int64_t o_row_stride, float* lse, float softmax_scale, void* stream);
 
+/* Chunked prefill (sec 2: time to first token gates decode batching, so a serving engine runs a long
+ * prompt in chunks between decode steps).  Rows [row_begin, row_end) of the packed token axis only:
+ * the same metadata, the same kernel and the same schedule as sift_prefill_attention, with M-blocks that have no row
+ * in the range skipped and tiles / rows outside it neither computed nor written.  O and lse are the full-size arrays
+ * of sift_prefill_attention (same base pointers and strides); rows outside the range keep what they held.  Every row
+ * in the range is bit-identical to what sift_prefill_attention writes for it (a row's steps and their order do not
+ * depend on which other rows run).
+ *   0 <= row_begin <= row_end <= N; an empty range launches nothing.  The range may cut tiles and documents anywhere;
+ *   whole tiles (multiples of `tile` inside a segment) waste no work.
+ *   K and V rows [0, E) must exist, E = min(N, first row of the last tile that intersects the range + 128): the copy
+ *   engine fetches 128-row boxes, so the box of that tile reaches past a ragged tile end and past row_end.  Keys at or
+ *   after a row's own position are masked, but V rows of a fetched box enter the MMAs with weight 0, so V rows
+ *   [row_end, E) must be finite (zeros will do; K and Q rows there may hold anything).  Rows >= E are never read.
+ * Same ordering rule: calls on one (metadata, layer) are stream-ordered, whole-prompt and ranged ones alike. */
+int sift_prefill_attention_rows(const sift_shape* shape, int32_t layer, int32_t row_begin, int32_t row_end,
+                                const void* Q, const void* K, const void* V,
+                                int64_t q_row_stride, int64_t k_row_stride, int64_t v_row_stride,
+                                const void* metadata /*dev*/, void* O, int64_t o_row_stride, float* lse,
+                                float softmax_scale, void* stream);
+
 /* FP8 variant (sec 2.6 points at FP8 prefill; reading R7).  Q8 [N][n_q_heads][128], K8, V8
  * [N][n_kv_heads][128]: OCP e4m3 bytes, dev, row strides in elements (= bytes), bases and strides 16-byte aligned;
  * q_scale HOST [n_q_heads], k_scale / v_scale HOST [n_kv_heads], all > 0.  The result is sift_prefill_attention of the

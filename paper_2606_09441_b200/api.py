@@ -18,7 +18,8 @@ EXPORTS = ("sift_version", "sift_last_error", "sift_metadata_size", "sift_metada
            "sift_encode_workspace_size", "sift_encode_output_sizes", "sift_encode_document",
            "sift_host_ctx_create", "sift_host_ctx_destroy", "sift_prefill_layer_host_workspace_size",
            "sift_prefill_layer_host", "sift_paper_index_offsets", "sift_export_paper_indices",
-           "sift_prefill_attention_fp8", "sift_encode_document_static", "sift_encode_static_scratch_bytes")
+           "sift_prefill_attention_fp8", "sift_encode_document_static", "sift_encode_static_scratch_bytes",
+           "sift_prefill_attention_rows")
 
 
 class SiftShape(C.Structure):
@@ -63,6 +64,8 @@ def lib() -> C.CDLL:
         L.sift_prefill_attention.argtypes = [C.POINTER(SiftShape), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                              C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_int64,
                                              C.c_void_p, C.c_float, C.c_void_p]
+        a = L.sift_prefill_attention.argtypes
+        L.sift_prefill_attention_rows.argtypes = a[:2] + [C.c_int32, C.c_int32] + a[2:]
         L.sift_dense_causal_attention.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
                                                   C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_int64,
                                                   C.c_void_p, C.c_float, C.c_void_p]
@@ -219,6 +222,19 @@ def sift_prefill_attention(shape: Shape, layer: int, q: torch.Tensor, k: torch.T
                                       float(softmax_scale), _stream(stream))
     _check(rc, "sift_prefill_attention")
     return out, lse
+
+
+def sift_prefill_attention_rows(shape: Shape, layer: int, row_begin: int, row_end: int, q: torch.Tensor, k: torch.Tensor,
+                                v: torch.Tensor, metadata: torch.Tensor, out: torch.Tensor,
+                                lse: Optional[torch.Tensor] = None, softmax_scale: float = 0.0, stream=None) -> None:
+    """Rows [row_begin, row_end) of sift_prefill_attention (chunked prefill): `out` [N, Hq, d] and `lse` [Hq, N] are the
+    full-size arrays, only the rows of the range are written."""
+    _check_qkv(q, k, v)
+    rc = lib().sift_prefill_attention_rows(C.byref(shape.c), layer, int(row_begin), int(row_end), q.data_ptr(), k.data_ptr(),
+                                           v.data_ptr(), q.stride(0), k.stride(0), v.stride(0), metadata.data_ptr(),
+                                           out.data_ptr(), out.stride(0), lse.data_ptr() if lse is not None else None,
+                                           float(softmax_scale), _stream(stream))
+    _check(rc, "sift_prefill_attention_rows")
 
 
 def sift_dense_causal_attention(q: torch.Tensor, k: torch.Tensor, v: torch.Tensor, out: Optional[torch.Tensor] = None,

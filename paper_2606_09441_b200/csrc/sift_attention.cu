@@ -9,7 +9,7 @@
 //     list, so every gathered K/V tile in shared memory feeds two accumulators;
 //   * warp roles: warp 13 = work-item fetch + Q tiles (TMA); warp 1 = tcgen05.mma issuer (warp-uniform operands, one
 //     elected lane issues); warps 2, 3, 14 = K producers, warps 0, 12, 15 = V producers (tiled TMA boxes for local tiles,
-//     pages and dense rows; TMA `tile::gather4`, or cp.async, for the row-granular cross keys); warps 4..11 = one softmax
+//     pages and dense rows; TMA `tile::gather4` for the row-granular cross keys); warps 4..11 = one softmax
 //     warpgroup per query tile (one row per thread, S read with tcgen05.ld, P written back to TMEM as bf16 in four key
 //     ranges and used as the A operand of the P*V MMAs, lazy rescale of the TMEM-resident O accumulator);
 //   * registers are re-split with setmaxnreg per sub-partition: softmax 216, MMA issuer 56, producers 40, item warp 24;
@@ -40,10 +40,10 @@ constexpr int kBN = 128;                    // keys per step
 #endif
 constexpr int kPvParts = SIFT_PV_PARTS;     // P V is issued in this many key ranges, each as soon as its P is written
 static_assert(kPvParts == 1 || kPvParts == 2 || kPvParts == 4, "P V parts");
-constexpr int kNumThreads = 256 + 128 * kNQ;        // warps 0-3 control/K, softmax warpgroups, 2 V-producer warps, 2 idle
+constexpr int kNumThreads = 256 + 128 * kNQ;        // 16 warps, every one with a role: V/MMA/K/K, two softmax warpgroups, V/item/K/V
                                                    // (4 warps per SM sub-partition: registers are pooled per sub-partition)
 constexpr int kFirstVWarp = 4 + 4 * kNQ;
-constexpr int kProducerThreads = 96;              // per operand: K = warps 2, 3, 14; V = warps 12, 13, 15
+constexpr int kProducerThreads = 96;              // per operand: K = warps 2, 3, 14; V = warps 0, 12, 15
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 with a stale max
 constexpr uint32_t kTmemCols = 512;
 
@@ -73,6 +73,10 @@ struct AttnParams {
   int32_t kv_per_group;     // dense comparator: kv heads scheduled together (sched_kv_heads_per_group)
   int32_t o_vec32;          // O rows are 32-byte aligned: the epilogue may use 256-bit stores
   int32_t paged;            // cross_gran == tile: cross entries are global tile ids, one tiled step each
+  int32_t row_lo, row_hi;   // only rows [row_lo, row_hi) are computed and written (sift_prefill_attention_rows; the whole
+                            // prompt: 0, n_tokens)
+  int32_t ranged;           // the range is a proper part: the item warp skips M-blocks outside [mb_lo, mb_hi)
+  int32_t mb_lo, mb_hi;
   __nv_bfloat16* o;
   int64_t o_row_stride;
   float* lse;  // [Hq][N] or null
@@ -169,10 +173,14 @@ __device__ __forceinline__ Item load_item(const AttnParams& p, int code) {
   }
 #pragma unroll
   for (int q = 0; q < kNQ; ++q) {
-    if (q < nt) {
-      it.tile_id[q] = t0 + q;
+    bool on = q < nt;
+    if (on) {
       it.row0[q] = p.tile_row0[t0 + q];
       it.rows[q] = p.tile_rows[t0 + q];
+      on = it.row0[q] < p.row_hi && it.row0[q] + it.rows[q] > p.row_lo;   // a tile outside the row range is absent
+    }
+    if (on) {
+      it.tile_id[q] = t0 + q;
       it.lptr[q] = p.local_ptr[lh * (p.n_tiles + 1) + t0 + q];
       it.lcnt[q] = p.local_cnt[lh * p.n_tiles + t0 + q];
     } else {
@@ -300,7 +308,7 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
     // ======================================= item fetch + Q producer =======================================
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsItem));
     const uint32_t q_smem = sbase + S::kQOff;
-    for (int it_n = 0;; ++it_n) {
+    for (int it_n = 0;;) {
       const int slot = it_n & 1;
       mbar_wait(bar(S::bItemEmpty + slot), ((it_n >> 1) & 1) ^ 1, 100);
       int code = -1;
@@ -315,14 +323,22 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
           } else {
             code = p.sched[idx];
           }
-        } else {
+        }
+        if (code < 0) {
           const int f = atomicAdd(&p.counters[1], 1);
           if (f == (int)gridDim.x - 1) { atomicExch(&p.counters[0], 0); atomicExch(&p.counters[1], 0); }
         }
+      }
+      code = __shfl_sync(0xffffffffu, code, 0);
+      // row-range call: M-blocks are numbered in token order, so the ones with rows in [row_lo, row_hi) are the index
+      // range [mb_lo, mb_hi) the host worked out; an item outside it is dropped here and the next one fetched into the
+      // same ring slot (one atomic + one load per skipped item, on this warp only: no other role sees a skipped item)
+      if (p.ranged && code >= 0 && ((code & 0xFFFFF) < p.mb_lo || (code & 0xFFFFF) >= p.mb_hi)) continue;
+      if (lane == 0) {
         info[1 + slot] = code;
         mbar_arrive(bar(S::bItemFull + slot));
       }
-      code = __shfl_sync(0xffffffffu, code, 0);
+      __syncwarp();
       if (code < 0) break;
       const Item it = load_item(p, code);
       {
@@ -355,6 +371,7 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
                         it.row0[q]);
       }
       __syncwarp();
+      ++it_n;
     }
   } else if (warp == 0 || warp == 2 || warp == 3 || (warp >= kFirstVWarp && warp != kItemWarp)) {
     // ======================================= K (warps 2,3) / V (last two warps) producers =======================================
@@ -425,7 +442,14 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
         const int ngroups = p.paged ? 0 : (it.cp - it.c0 + kBN - 1) / kBN;
         if (p.paged) {                     // page-granular cross keys: the listed pages as tiled boxes
           const int32_t* cidx = p.cross_idx + (int64_t)it.h * p.cross_cap;
-          for (int e = it.c0; e < it.cp; ++e) emit(false, p.tile_row0[cidx[e]], present, e == it.cp - 1 && nloc == 0);
+          // the page's first row is two dependent loads away (entry -> tile_row0): fetched one step ahead, so that the
+          // latency runs under the wait for the stage instead of in front of every TMA issue
+          int row_next = it.c0 < it.cp ? p.tile_row0[cidx[it.c0]] : 0;
+          for (int e = it.c0; e < it.cp; ++e) {
+            const int row = row_next;
+            if (e + 1 < it.cp) row_next = p.tile_row0[cidx[e + 1]];
+            emit(false, row, present, e == it.cp - 1 && nloc == 0);
+          }
         }
         for (int g = 0; g < ngroups; ++g) emit(true, it.c0 + g * kBN, present, g == ngroups - 1 && nloc == 0);
         const int32_t* lidx = p.local_idx + (int64_t)it.h * p.local_cap;
@@ -590,9 +614,16 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
         if constexpr (kF8) sl = f8->qk_log2[h];
       }
       float m = -INFINITY, l = 0.f;
+      // page-granular cross steps: the valid rows of the page (a document's last page may be ragged) are two dependent
+      // loads away; the pair for step e + 1 is issued at the top of step e, so its latency runs under this step's work
+      const int32_t* pg_idx = p.cross_idx + (int64_t)h * p.cross_cap + c0;
+      int pg_lim = (paged_item && ngroups > 0) ? p.tile_rows[pg_idx[0]] : kBN;
       for (int e = 0; e < nsteps; ++e, lim -= kBN) {
         int cur_lim = (e < ngroups) ? lim : (e == diag_step ? min(tile_lim, r + 1) : tile_lim);
-        if (paged_item && e < ngroups) cur_lim = p.tile_rows[p.cross_idx[(int64_t)h * p.cross_cap + c0 + e]];   // a page may be ragged
+        if (paged_item && e < ngroups) {
+          cur_lim = pg_lim;
+          if (e + 1 < ngroups) pg_lim = p.tile_rows[pg_idx[e + 1]];
+        }
         mbar_wait(bar(S::bSFull + q), sph, 301);
         sph ^= 1;
         tc_fence_after();
@@ -713,7 +744,7 @@ __device__ __forceinline__ void sift_attention_body(const CUtensorMap& tm_q, con
       }
       // ---- epilogue: O / l -> bf16, LSE
       const int64_t grow = (int64_t)row0 + r;
-      const bool row_ok = r < rows;
+      const bool row_ok = r < rows && grow >= p.row_lo && grow < p.row_hi;
       __nv_bfloat16* orow = p.o + grow * p.o_row_stride + (int64_t)h * HD;
       if (nsteps > 0) {
         mbar_wait(bar(S::bODone + q), (pv_cnt - 1) & 1, 303);
@@ -848,6 +879,7 @@ static int sparse_params(const sift_shape* shape, int32_t layer, const void* met
   p.n_tokens = lay.n_tokens;
   p.n_q_heads = Hq; p.n_kv_heads = shape->n_kv_heads; p.tile = shape->tile;
   p.paged = (shape->cross_gran != 1);
+  p.row_lo = 0; p.row_hi = lay.n_tokens; p.ranged = 0;
   p.o = static_cast<__nv_bfloat16*>(O); p.o_row_stride = o_row_stride; p.lse = lse;
   p.o_vec32 = (((uintptr_t)O & 31) == 0 && (o_row_stride * 2) % 32 == 0);
   const float sc = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf((float)HD);
@@ -869,6 +901,49 @@ extern "C" int sift_prefill_attention(const sift_shape* shape, int32_t layer, co
   if (q_row_stride < (int64_t)Hq * HD || k_row_stride < (int64_t)shape->n_kv_heads * HD ||
       v_row_stride < (int64_t)shape->n_kv_heads * HD)
     return set_error(SIFT_ERR_INVALID_ARG, "row stride smaller than heads*head_dim");
+  if (HD == 128) return launch_attention<128>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
+  return launch_attention<64>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
+}
+
+extern "C" int sift_prefill_attention_rows(const sift_shape* shape, int32_t layer, int32_t row_begin, int32_t row_end,
+                                           const void* Q, const void* K, const void* V, int64_t q_row_stride,
+                                           int64_t k_row_stride, int64_t v_row_stride, const void* metadata, void* O,
+                                           int64_t o_row_stride, float* lse, float softmax_scale, void* stream) {
+  AttnParams p;
+  int rc = sparse_params(shape, layer, metadata, O, o_row_stride, lse, softmax_scale, &p);
+  if (rc) return rc;
+  if (row_begin < 0 || row_end > p.n_tokens || row_begin > row_end)
+    return set_error(SIFT_ERR_INVALID_ARG, "row range [%d, %d) not inside [0, %d)", row_begin, row_end, p.n_tokens);
+  if ((rc = check_tensor(Q, q_row_stride, "Q")) || (rc = check_tensor(K, k_row_stride, "K")) ||
+      (rc = check_tensor(V, v_row_stride, "V")))
+    return rc;
+  const int Hq = shape->n_q_heads, HD = shape->head_dim;
+  if (q_row_stride < (int64_t)Hq * HD || k_row_stride < (int64_t)shape->n_kv_heads * HD ||
+      v_row_stride < (int64_t)shape->n_kv_heads * HD)
+    return set_error(SIFT_ERR_INVALID_ARG, "row stride smaller than heads*head_dim");
+  if (row_begin == row_end) return SIFT_OK;      // nothing to compute, nothing launched
+  p.row_lo = row_begin; p.row_hi = row_end;
+  p.ranged = !(row_begin == 0 && row_end == p.n_tokens);
+  {
+    // M-blocks (kNQ tiles of one segment, numbered in token order as compute_layout counts them) that hold a row of
+    // the range
+    static thread_local DocTable dt;
+    build_segments(shape, &dt);
+    const int64_t rows_mb = (int64_t)shape->tile * kNQ;
+    int64_t mb = 0;
+    p.mb_lo = -1; p.mb_hi = 0;
+    for (int sg = 0; sg < dt.n_seg; ++sg) {
+      const int64_t a = dt.off[sg], b = dt.off[sg + 1], n_mb = (b - a + rows_mb - 1) / rows_mb;
+      if (b > row_begin && a < row_end && b > a) {
+        const int64_t lo = row_begin > a ? (row_begin - a) / rows_mb : 0;
+        const int64_t hi = row_end < b ? (row_end - a + rows_mb - 1) / rows_mb : n_mb;   // first M-block past the range
+        if (p.mb_lo < 0) p.mb_lo = (int32_t)(mb + lo);
+        p.mb_hi = (int32_t)(mb + hi);
+      }
+      mb += n_mb;
+    }
+    if (p.mb_lo < 0) p.mb_lo = 0;
+  }
   if (HD == 128) return launch_attention<128>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
   return launch_attention<64>(p, Q, K, V, q_row_stride, k_row_stride, v_row_stride, (cudaStream_t)stream);
 }
@@ -915,6 +990,7 @@ extern "C" int sift_dense_causal_attention(int32_t n_tokens, int32_t n_q_heads, 
   memset(&p, 0, sizeof(p));
   p.dense = 1;
   p.n_tokens = n_tokens; p.n_q_heads = n_q_heads; p.n_kv_heads = n_kv_heads; p.tile = 128;
+  p.row_lo = 0; p.row_hi = n_tokens;
   p.n_mblocks = (n_tokens + kBM * kNQ - 1) / (kBM * kNQ);
   p.kv_per_group = sched_kv_heads_per_group(n_tokens, head_dim, n_kv_heads);
   p.n_items = p.n_mblocks * n_q_heads;

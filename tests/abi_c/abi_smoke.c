@@ -52,6 +52,23 @@ static int host_part(void) {
   off[2] = 500;
   CHECK(sift_prefill_layer_host_workspace_size(&s, 100, 100, &nb) == SIFT_OK && nb > 2u * 570u * 4u * 128u * 2u);
   CHECK(sift_prefill_layer_host(NULL, &s, 0, NULL, 0, NULL, NULL, 0, NULL, NULL, NULL, NULL, 0, 0, 0, NULL, 0, NULL, 0.f, NULL, 0, NULL) == SIFT_ERR_INVALID_ARG);
+  /* a caller built against the header before the prompt fields: a shape of SIFT_SHAPE_SIZE_V1 bytes (poison behind it)
+   * and a sift_md_layout that ends before n_seg; the library reads / writes no further than that */
+  {
+    unsigned char sbuf[sizeof(sift_shape) + 32], obuf[sizeof(sift_md_layout) + 32];
+    sift_md_layout full, v1;
+    size_t nb1 = 0;
+    CHECK(sift_metadata_layout(&s, &full) == SIFT_OK && full.struct_size == sizeof(sift_md_layout));
+    memset(sbuf, 0xCD, sizeof(sbuf)); memset(obuf, 0xAB, sizeof(obuf));
+    memcpy(sbuf, &s, SIFT_SHAPE_SIZE_V1);
+    ((sift_shape*)sbuf)->struct_size = SIFT_SHAPE_SIZE_V1;
+    CHECK(sift_metadata_layout((const sift_shape*)sbuf, (sift_md_layout*)obuf) == SIFT_OK);
+    for (size_t i = SIFT_MD_LAYOUT_SIZE_V1; i < sizeof(obuf); ++i) CHECK(obuf[i] == 0xAB);
+    memcpy(&v1, obuf, SIFT_MD_LAYOUT_SIZE_V1);
+    CHECK(v1.struct_size == SIFT_MD_LAYOUT_SIZE_V1 && v1.total_bytes == full.total_bytes && v1.counters == full.counters &&
+          v1.n_items == full.n_items);
+    CHECK(sift_metadata_size((const sift_shape*)sbuf, &nb1) == SIFT_OK && nb1 == full.total_bytes);
+  }
   printf("abi_smoke host ok\n");
   return 0;
 }
@@ -134,6 +151,19 @@ static int gpu_part(void) {
     CHECK(sift_host_ctx_destroy(ctx) == SIFT_OK);
     cudaStreamDestroy(st); cudaFree(d_ws);
     cudaFreeHost(p_la); cudaFreeHost(p_ca); cudaFreeHost(p_q); cudaFreeHost(p_k); cudaFreeHost(p_v); cudaFreeHost(p_o); cudaFreeHost(p_lse);
+  }
+  /* chunked prefill: the prompt in three row ranges that cut a tile, a document and the query; O / LSE start poisoned
+   * and must end bit-identical to the single call; a range that reaches past N is refused */
+  {
+    const int cut[4] = {0, 100, 333, N};
+    CHECK(cudaMemset(d_o, 0xff, qb) == 0 && cudaMemset(d_lse, 0xff, (size_t)HQ * N * 4) == 0);
+    for (int c = 0; c < 3; ++c)
+      CHECK(sift_prefill_attention_rows(&s, 0, cut[c], cut[c + 1], d_q, d_k, d_v, HQ * D, HKV * D, HKV * D, d_md, d_o, HQ * D,
+                                        (float*)d_lse, 0.f, NULL) == SIFT_OK);
+    CHECK(cudaDeviceSynchronize() == 0 && cudaMemcpy(ho, d_o, qb, 2) == 0 && cudaMemcpy(hl, d_lse, (size_t)HQ * N * 4, 2) == 0);
+    CHECK(memcmp(ho, ho_sparse, qb) == 0 && memcmp(hl, hl_sparse, (size_t)HQ * N * 4) == 0);
+    CHECK(sift_prefill_attention_rows(&s, 0, 10, N + 1, d_q, d_k, d_v, HQ * D, HKV * D, HKV * D, d_md, d_o, HQ * D, NULL, 0.f, NULL) ==
+          SIFT_ERR_INVALID_ARG);
   }
   /* two prompts in one call (sift_shape.n_prompts): the same prompt twice, packed back to back; every row must see its own
    * prompt only, i.e. both halves of O and LSE repeat the single-prompt result bit for bit.  Then the paper's index layout. */
