@@ -141,10 +141,11 @@ int sift_prefill_attention(const sift_shape* shape, int32_t layer,
  * depend on which other rows run).
  *   0 <= row_begin <= row_end <= N; an empty range launches nothing.  The range may cut tiles and documents anywhere;
  *   whole tiles (multiples of `tile` inside a segment) waste no work.
- *   K and V rows [0, E) must exist, E = min(N, first row of the last tile that intersects the range + 128): the copy
- *   engine fetches 128-row boxes, so the box of that tile reaches past a ragged tile end and past row_end.  Keys at or
- *   after a row's own position are masked, but V rows of a fetched box enter the MMAs with weight 0, so V rows
- *   [row_end, E) must be finite (zeros will do; K and Q rows there may hold anything).  Rows >= E are never read.
+ *   K and V rows [0, E) must exist, E = min(N, e + 127), e = one past the last row of the last tile that intersects
+ *   the range: the copy engine fetches 128-row boxes (a document tile's box starts at the tile, a query tile's boxes
+ *   at multiples of 128 from its prompt's first row), so the last box reaches past a ragged tile end and past row_end.
+ *   Keys at or after a row's own position are masked, but V rows of a fetched box enter the MMAs with weight 0, so V
+ *   rows [row_end, E) must be finite (zeros will do; K and Q rows there may hold anything).  Rows >= E are never read.
  * Same ordering rule: calls on one (metadata, layer) are stream-ordered, whole-prompt and ranged ones alike. */
 int sift_prefill_attention_rows(const sift_shape* shape, int32_t layer, int32_t row_begin, int32_t row_end,
                                 const void* Q, const void* K, const void* V,

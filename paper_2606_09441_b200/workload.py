@@ -305,14 +305,14 @@ def ragged_doc_lens(seed: int, n_docs: int = 24, lo: int = 1024, hi: int = 4096,
     return tuple(out)
 
 
-def config_64k_ragged(seed: int = BASE_SEED) -> Workload:
+def config_64k_ragged(seed: int = BASE_SEED, cross_gran: int = 1) -> Workload:
     lens = ragged_doc_lens(seed)
-    sh = PromptShape(1, 32, 8, 128, lens, 512, tile=128, cross_gran=1)
+    sh = PromptShape(1, 32, 8, 128, lens, 512, tile=128, cross_gran=cross_gran)
     pl, pc = _beta_dens(seed, 1, 32)
     r = _rng(seed, _S_SCALE)
     qs = r.lognormal(0.0, 0.5, (1, 32))
     ks = r.lognormal(0.0, 0.5, (1, 8))
-    return build_workload("C4-64k-ragged", sh, seed, pl, pc, q_scale=qs, k_scale=ks,
+    return build_workload("C4-64k-ragged" + ("" if cross_gran == 1 else "-paged"), sh, seed, pl, pc, q_scale=qs, k_scale=ks,
                           recipe="24 docs U[1024,4096] clipped to <=65536 incl. 512 query; Beta densities; "
                                  "Q/K scaled per head by LogNormal(0,.5)")
 

@@ -48,14 +48,14 @@ def test_chunks_are_bit_identical_and_match_the_oracle(gran):
 
 
 def test_chunk_needs_no_keys_past_its_last_tile():
-    """Chunked prefill proper: when a chunk runs, K / V / Q of later rows do not exist yet.  Rows from E = first row of
-    the chunk's last tile + 128 (the copy engine's box; include/sift.h) are NaN here, K and Q already from row_end, and
-    the chunk still equals the whole-prompt result."""
+    """Chunked prefill proper: when a chunk runs, K / V / Q of later rows do not exist yet.  Rows from E = (end of the
+    chunk's last tile) + 127 (the reach of the copy engine's last 128-row box; include/sift.h) are NaN here, K and Q
+    already from row_end, and the chunk still equals the whole-prompt result."""
     w, shape, md, q, k, v = _prompt("chunked-nan", n_q_heads=4, n_kv_heads=2, head_dim=128, doc_lens=(700, 900), query_len=333,
                                     tile=128, p_cross=0.5, seed=92)
     o_ref, lse_ref = api.sift_prefill_attention(shape, 0, q, k, v, md)
     n = q.shape[0]
-    for a, b, e in ((0, 600, 640), (600, 700, 640 + 128), (700, 1000, 700 + 384), (1600, 1700, 1600 + 128)):
+    for a, b, e in ((0, 600, 640 + 127), (600, 700, 700 + 127), (700, 1000, 1084 + 127), (1600, 1700, 1728 + 127)):
         q2, k2, v2 = q.clone(), k.clone(), v.clone()
         for t in (q2, k2):
             t[b:] = float("nan")
