@@ -1,6 +1,8 @@
 """-m gpu parity at full size for the widened rows of SURVEY.md 8(f), at the sizes bench.py times them (VERDICT r2,
 weak 8): page-granular CA on C3 and C4 (every head, a row in every query tile + tails + boundaries), e4m3 Q/K/V on C3
-and C4 (the same rows; the measured errors are printed beside the bound), the encoder on the benched 2000-token document
+and C4 (the same rows on a subset of heads that covers every kv head -- the e4m3 oracle is slow: all 32 heads of both took
+12 of the suite's 19 minutes in the r3 builder run, where they measured max-abs 4.4e-2 / mean-abs 2.3e-3; the measured
+errors are printed beside the bound, which is 2x those figures for this test), the encoder on the benched 2000-token document
 and on 4096 tokens, and the TP = 8 head split of C2 bit-identical to the unsharded call."""
 import numpy as np
 import pytest
@@ -26,14 +28,20 @@ def test_paged_every_head_every_tile(cfg):
            gu.attention_errors(w, 0, o, lse, range(w.shape.n_q_heads), rows_one_per_tile(w)))
 
 
-@pytest.mark.parametrize("cfg", ["32k", "64k-ragged"])
-def test_fp8_every_head_every_tile(cfg):
+# 2x the worst error measured on all 32 heads of C3 and C4 (r3 builder run: 4.38e-2 / 2.28e-3); DESIGN.md's derivation
+# (TOL8_MAX, TOL8_MEAN) stays the upper bound for the small cases
+FULL8_MAX, FULL8_MEAN = 0.09, 5e-3
+assert FULL8_MAX <= TOL8_MAX and FULL8_MEAN <= TOL8_MEAN
+
+
+@pytest.mark.parametrize("cfg,heads", [("32k", range(0, 32, 2)), ("64k-ragged", range(1, 32, 4))])
+def test_fp8_every_kv_head_every_tile(cfg, heads):
     w = wl.CONFIGS[cfg]()
     packed, o, lse = fp8_run(w)
     assert torch.isfinite(o).all()
-    mx, mean, le = fp8_errors(w, 0, packed, o, lse, range(w.shape.n_q_heads), rows_one_per_tile(w))
-    print(f"[parity-full] fp8 {cfg}: max_abs={mx:.3e} (bound {TOL8_MAX}) mean_abs={mean:.3e} (bound {TOL8_MEAN}) lse={le:.3e}")
-    assert mx <= TOL8_MAX and mean <= TOL8_MEAN and le <= gu.TOL_LSE, (mx, mean, le)
+    mx, mean, le = fp8_errors(w, 0, packed, o, lse, heads, rows_one_per_tile(w))
+    print(f"[parity-full] fp8 {cfg} heads {list(heads)}: max_abs={mx:.3e} (bound {FULL8_MAX}) mean_abs={mean:.3e} (bound {FULL8_MEAN}) lse={le:.3e}")
+    assert mx <= FULL8_MAX and mean <= FULL8_MEAN and le <= gu.TOL_LSE, (mx, mean, le)
 
 
 @pytest.mark.parametrize("case", [
